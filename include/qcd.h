@@ -1,0 +1,131 @@
+/*
+ * qcd.h -- C ABI of the B200-native staggered-fermion hot path of arXiv:1710.09178
+ * (Gupta & Majumdar): the even-odd staggered Dirac operator D_oe / D_eo, the
+ * single-parity normal operator (M^dag M)_pp = m^2 - D_pq D_qp, and the multishift
+ * conjugate gradient that evaluates the partial-fraction sum of the rational
+ * approximation (eq. 8).  Citations are PAPER.md:<line>; "SURVEY C<n>" names a
+ * reading of the paper listed in SURVEY.md 8(c) and DESIGN.md.
+ *
+ * Conventions
+ * -----------
+ *  Lattice     sites x = (x,y,z,t), 0 <= x_mu < N_mu, all N_mu even and >= 2.
+ *              canonical address l = ((t*Nz + z)*Ny + y)*Nx + x        (PAPER.md:43, 0-based)
+ *              parity(x) = (x+y+z+t) mod 2, QCD_EVEN = 0                (Fig. 2; C2)
+ *  Operator    (D psi)(x) = 1/2 sum_mu eta_mu(x) [ s+ U_mu(x) psi(x+mu) - s- U_mu(x-mu)^dag psi(x-mu) ]
+ *              (PAPER.md:106 in the M = m + D normalisation, C1), eta_0 = 1, eta_1 = (-1)^x,
+ *              eta_2 = (-1)^(x+y), eta_3 = (-1)^(x+y+z) (C4); periodic in x,y,z, antiperiodic
+ *              in t: s+ = -1 on the hop t = Nt-1 -> 0, s- = -1 on the hop t = 0 -> Nt-1 (C5).
+ *  Canonical layouts (what callers exchange; fp64, little-endian, (re,im) pairs):
+ *              links          double[V][4][3][3][2] = U_mu(l)[row][col]     72 V doubles
+ *              parity vector  double[V/2][3][2], the sites of ONE parity in increasing l
+ *                             (a full colour vector is 6 V doubles)
+ *  Internal layout            the library's own parity-split, site-fastest SoA ("ap(V,3)",
+ *              PAPER.md:210): an internal vector is 6*(V/2) doubles, opaque to the caller;
+ *              qcd_pack / qcd_unpack convert.  All internal vectors must be 16-byte aligned.
+ *  Pointers    d_* = DEVICE memory owned by the caller (e.g. torch.empty(...).data_ptr());
+ *              h_* = HOST memory owned by the caller.  The library owns only its handle, its
+ *              reordered gauge copy and its workspace, all released by qcd_destroy.
+ *              No pointer is retained after a call returns.
+ *  Streams     all work is enqueued on the context's stream.  qcd_dslash, qcd_mdagm, qcd_pack,
+ *              qcd_unpack, qcd_load_gauge return WITHOUT synchronising.  Calls that return host
+ *              scalars or fill host buffers (qcd_multishift_cg, *_host) synchronise the stream
+ *              before returning.
+ *  Errors      every call returns a qcd_status; nothing aborts or throws across the ABI.
+ *              qcd_last_error() gives the text of the last failure on that context (or of the
+ *              last failed qcd_create when ctx == NULL).
+ *  No CPU fallback: without an sm_100 CUDA device qcd_create returns QCD_ECUDA.
+ */
+#ifndef QCD_H
+#define QCD_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QCD_API __attribute__((visibility("default")))
+
+typedef struct qcd_ctx qcd_ctx; /* opaque; owned by the library */
+
+typedef enum {
+    QCD_OK = 0,
+    QCD_EINVAL = 1,   /* bad argument: odd or < 2 extent, NULL pointer, negative shift, nshift < 1 or
+                         > QCD_MAX_SHIFTS, tol <= 0, bad parity, aliasing in/out */
+    QCD_ENOMEM = 2,   /* device or host allocation failed */
+    QCD_ECUDA = 3,    /* CUDA error, or no sm_100 device */
+    QCD_ENOTCONV = 4, /* max_iter reached; outputs are still written and true_res filled */
+    QCD_ESTATE = 5    /* operator used before qcd_load_gauge */
+} qcd_status;
+
+enum { QCD_EVEN = 0, QCD_ODD = 1 };
+enum { QCD_MAX_SHIFTS = 64 };
+
+/* Library version string, e.g. "qcd_b200 0.1 (sm_100a)". */
+QCD_API const char *qcd_version(void);
+
+/* Create a context for an Nx x Ny x Nz x Nt lattice (dims = {Nx,Ny,Nz,Nt}) and quark mass m.
+ * cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the
+ * default stream.  Uses the calling thread's current CUDA device. */
+QCD_API qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx **out);
+QCD_API qcd_status qcd_destroy(qcd_ctx *ctx);
+QCD_API qcd_status qcd_set_mass(qcd_ctx *ctx, double mass);
+QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
+
+/* Size in doubles of one internal parity vector: 6 * V/2. */
+QCD_API long qcd_vector_doubles(const qcd_ctx *ctx);
+
+/* a1: ingest the gauge field.  d_links_canonical: 72*V doubles, canonical layout.
+ * Builds the library's parity-split site-fastest copy with 1/2, eta_mu(x) and the antiperiodic
+ * sign folded into the stored links ("certain phases have been absorbed into the U's",
+ * PAPER.md:104).  The caller's buffer is not retained. */
+QCD_API qcd_status qcd_load_gauge(qcd_ctx *ctx, const double *d_links_canonical);
+QCD_API qcd_status qcd_load_gauge_host(qcd_ctx *ctx, const double *h_links_canonical);
+
+/* Canonical one-parity vector (6*V/2 doubles) <-> internal vector.  in/out must not alias. */
+QCD_API qcd_status qcd_pack(qcd_ctx *ctx, int parity, const double *d_canonical, double *d_internal);
+QCD_API qcd_status qcd_unpack(qcd_ctx *ctx, int parity, const double *d_internal, double *d_canonical);
+
+/* a2/a3: d_out[out_parity] = D_{out_parity, other} d_in[other]  (C6):
+ * out_parity = QCD_ODD is D_oe (even in, odd out), QCD_EVEN is D_eo.  Internal layout; d_in and
+ * d_out must not alias. */
+QCD_API qcd_status qcd_dslash(qcd_ctx *ctx, int out_parity, const double *d_in, double *d_out);
+
+/* a4: d_out = m^2 d_in - D_{p,q} D_{q,p} d_in on `parity` p  (C3).
+ * Internal layout; d_in and d_out must not alias. */
+QCD_API qcd_status qcd_mdagm(qcd_ctx *ctx, int parity, const double *d_in, double *d_out);
+
+/* a5/a6: multishift CG (refs [5],[6]; recurrences SURVEY 8(c.2)).  Solves
+ * (M^dag M + shifts[k]) x_k = d_b on `parity` for k < nshift, x_k = 0 initial guess (C11), until the
+ * base (smallest-shift) system's recursion residual satisfies ||r|| <= tol ||b|| (C10); converged
+ * shifts are frozen at 0.1 tol (C13).  Shifts need not be sorted (C12).
+ *   d_b        internal vector (source)
+ *   shifts     host, nshift values >= 0;   residues: host, nshift values (c_k of eq. 8)
+ *   d_x        nshift internal vectors, contiguous, caller's shift order; may be NULL
+ *   d_y        internal vector, y = sum_k residues[k] x_k (eq. 8 without c_0, C14); may be NULL
+ *   iterations host int;  true_res: host, nshift doubles, ||b - (M^dag M + sigma_k) x_k|| / ||b||
+ *              recomputed from x_k (not the recursion value).
+ * Returns QCD_OK, or QCD_ENOTCONV if max_iter iterations did not reach tol. Synchronises. */
+QCD_API qcd_status qcd_multishift_cg(qcd_ctx *ctx, int parity, const double *d_b, int nshift,
+                             const double *shifts, const double *residues, double tol,
+                             int max_iter, double *d_x, double *d_y, int *iterations,
+                             double *true_res);
+
+/* Host-buffer forms (canonical layout on the host; H2D copy, pack, compute, unpack, D2H copy and a
+ * stream synchronise all happen inside the call).  h_x: nshift canonical parity vectors or NULL;
+ * h_y: one canonical parity vector or NULL. */
+QCD_API qcd_status qcd_dslash_host(qcd_ctx *ctx, int out_parity, const double *h_in, double *h_out);
+QCD_API qcd_status qcd_mdagm_host(qcd_ctx *ctx, int parity, const double *h_in, double *h_out);
+QCD_API qcd_status qcd_multishift_cg_host(qcd_ctx *ctx, int parity, const double *h_b, int nshift,
+                                  const double *shifts, const double *residues, double tol,
+                                  int max_iter, double *h_x, double *h_y, int *iterations,
+                                  double *true_res);
+
+/* Number of kernels this context has launched so far (for bench.py's gpu_launches claim). */
+QCD_API long qcd_launch_count(const qcd_ctx *ctx);
+
+/* Text of the last error on ctx (ctx == NULL: of the last failed qcd_create). Never NULL. */
+QCD_API const char *qcd_last_error(const qcd_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QCD_H */

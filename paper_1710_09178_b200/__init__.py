@@ -1,0 +1,12 @@
+"""B200-native staggered Dslash / M^dag M / multishift CG (arXiv:1710.09178 hot path).
+
+The product is the C-ABI library `libqcd_b200.so` (include/qcd.h, csrc/*.cu);
+this package is its thin ctypes binding: argument marshalling only.  There is no
+CPU fallback: importing works anywhere, but every call needs the built library
+and an sm_100 device, and fails loudly otherwise.
+"""
+from .binding import (QCD_EVEN, QCD_ODD, QcdError, Context, library_path, load_library,  # noqa: F401
+                      exported_symbols)
+
+__all__ = ["QCD_EVEN", "QCD_ODD", "QcdError", "Context", "library_path", "load_library",
+           "exported_symbols"]

@@ -1,0 +1,444 @@
+// api.cu -- the C ABI of include/qcd.h: context, argument checking, workspace, and the host-side
+// driver of the multishift CG (enqueue-only inside the iteration loop; the host only polls a pinned
+// copy of the device's `done` flag once per batch, lagged by one batch, to stop enqueuing).
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "internal.cuh"
+
+using namespace qcd;
+
+struct qcd_ctx {
+    Geom g{};
+    double mass = 0.0;
+    cudaStream_t stream = nullptr;
+    int device = 0;
+    long n2 = 0;              // double2 elements per internal vector = 3*Vh
+    size_t vec_bytes = 0;     // bytes of one parity vector (either layout)
+    double2 *W = nullptr;     // [2][4][9][Vh]
+    bool gauge_loaded = false;
+    // workspace (grow-only, freed by qcd_destroy)
+    double2 *tmp = nullptr, *q = nullptr, *r = nullptr;
+    double2 *p = nullptr;  int p_cap = 0;
+    double2 *xws = nullptr; int x_cap = 0;
+    double *partial = nullptr;
+    CgState *st = nullptr;
+    double *results = nullptr;          // device, kMaxShifts doubles
+    CgState *h_state = nullptr;         // pinned
+    int *h_done = nullptr;              // pinned [2]
+    double *h_results = nullptr;        // pinned
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    // staging for the *_host entry points
+    double *stage_links = nullptr;      // canonical gauge field on device
+    double *stage_vec = nullptr;        // one canonical parity vector on device
+    double2 *hv_a = nullptr, *hv_b = nullptr, *hv_y = nullptr;   // internal vectors
+    long launches = 0;
+    std::string err;
+};
+
+static std::string g_create_err;
+
+namespace {
+
+qcd_status fail(qcd_ctx *c, qcd_status s, const std::string &msg)
+{
+    if (c) c->err = msg; else g_create_err = msg;
+    return s;
+}
+
+#define QCD_CUDA(ctx, call)                                                                    \
+    do {                                                                                       \
+        cudaError_t e_ = (call);                                                               \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(ctx, e_ == cudaErrorMemoryAllocation ? QCD_ENOMEM : QCD_ECUDA,         \
+                        std::string(#call) + ": " + cudaGetErrorString(e_));                   \
+    } while (0)
+
+template <class T>
+cudaError_t dev_alloc(T **p, size_t count) { return cudaMalloc((void **)p, count * sizeof(T)); }
+
+qcd_status check_launch(qcd_ctx *c, const char *what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(c, QCD_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    return QCD_OK;
+}
+
+bool bad_parity(int p) { return p != QCD_EVEN && p != QCD_ODD; }
+
+qcd_status ensure_host_staging(qcd_ctx *c)
+{
+    if (!c->stage_vec) QCD_CUDA(c, cudaMalloc((void **)&c->stage_vec, c->vec_bytes));
+    if (!c->hv_a) QCD_CUDA(c, dev_alloc(&c->hv_a, (size_t)c->n2));
+    if (!c->hv_b) QCD_CUDA(c, dev_alloc(&c->hv_b, (size_t)c->n2));
+    return QCD_OK;
+}
+
+qcd_status ensure_cg_workspace(qcd_ctx *c, int nshift, bool need_x)
+{
+    if (!c->q) QCD_CUDA(c, dev_alloc(&c->q, (size_t)c->n2));
+    if (!c->r) QCD_CUDA(c, dev_alloc(&c->r, (size_t)c->n2));
+    if (c->p_cap < nshift) {
+        if (c->p) cudaFree(c->p);
+        c->p = nullptr; c->p_cap = 0;
+        QCD_CUDA(c, dev_alloc(&c->p, (size_t)c->n2 * nshift));
+        c->p_cap = nshift;
+    }
+    if (need_x && c->x_cap < nshift) {
+        if (c->xws) cudaFree(c->xws);
+        c->xws = nullptr; c->x_cap = 0;
+        QCD_CUDA(c, dev_alloc(&c->xws, (size_t)c->n2 * nshift));
+        c->x_cap = nshift;
+    }
+    return QCD_OK;
+}
+
+// out = D_{out_parity,other} in, with optional epilogue; counts the launch
+qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *out,
+                      const double2 *src, double coeff, bool coeff_from_state, int dot_mode,
+                      bool gated)
+{
+    DslashParams p{};
+    p.W = c->W; p.in = in; p.out = out; p.out_parity = out_parity;
+    p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
+    p.mass2 = c->mass * c->mass;
+    p.dot_mode = dot_mode; p.partial = c->partial;
+    p.st = (gated || dot_mode || coeff_from_state) ? c->st : nullptr;
+    c->launches += launch_dslash(c->g, p, c->stream);
+    return QCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *qcd_version(void) { return "qcd_b200 0.1 (sm_100a)"; }
+
+qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx **out)
+{
+    if (!out) return fail(nullptr, QCD_EINVAL, "qcd_create: out is NULL");
+    *out = nullptr;
+    if (!dims) return fail(nullptr, QCD_EINVAL, "qcd_create: dims is NULL");
+    for (int i = 0; i < 4; ++i)
+        if (dims[i] < 2 || (dims[i] & 1))
+            return fail(nullptr, QCD_EINVAL, "qcd_create: every extent must be even and >= 2");
+    if (!(mass == mass)) return fail(nullptr, QCD_EINVAL, "qcd_create: mass is NaN");
+    const long long V = 1LL * dims[0] * dims[1] * dims[2] * dims[3];
+    if (V / 2 * 72 >= (1LL << 31))
+        return fail(nullptr, QCD_EINVAL, "qcd_create: lattice too large for 32-bit link indexing");
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess)
+        return fail(nullptr, QCD_ECUDA, std::string("qcd_create: no CUDA device: ") + cudaGetErrorString(e));
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess)
+        return fail(nullptr, QCD_ECUDA, std::string("qcd_create: ") + cudaGetErrorString(e));
+    if (prop.major != 10)
+        return fail(nullptr, QCD_ECUDA, "qcd_create: device is not sm_100 (B200); there is no fallback path");
+
+    qcd_ctx *c = new (std::nothrow) qcd_ctx;
+    if (!c) return fail(nullptr, QCD_ENOMEM, "qcd_create: host allocation failed");
+    c->device = dev;
+    c->mass = mass;
+    c->stream = (cudaStream_t)cuda_stream;
+    Geom &g = c->g;
+    g.Nx = dims[0]; g.Ny = dims[1]; g.Nz = dims[2]; g.Nt = dims[3];
+    g.Nxh = g.Nx / 2;
+    g.Vh = (int)(V / 2);
+    g.sy = g.Nxh; g.sz = g.Nxh * g.Ny; g.st = g.Nxh * g.Ny * g.Nz;
+    g.dxh.init(g.Nxh); g.dy.init(g.Ny); g.dz.init(g.Nz);
+    c->n2 = 3L * g.Vh;
+    c->vec_bytes = (size_t)c->n2 * sizeof(double2);
+
+    auto cleanup = [&](qcd_status s, const std::string &m) { qcd_destroy(c); return fail(nullptr, s, m); };
+    const int nblk = std::max(dslash_grid_blocks(g), blas_grid_blocks(c->n2));
+    if (dev_alloc(&c->W, (size_t)72 * g.Vh) != cudaSuccess ||
+        dev_alloc(&c->tmp, (size_t)c->n2) != cudaSuccess ||
+        dev_alloc(&c->partial, (size_t)nblk) != cudaSuccess ||
+        dev_alloc(&c->st, 1) != cudaSuccess ||
+        dev_alloc(&c->results, (size_t)kMaxShifts + 1) != cudaSuccess)
+        return cleanup(QCD_ENOMEM, "qcd_create: device allocation failed");
+    if (cudaMallocHost((void **)&c->h_state, sizeof(CgState)) != cudaSuccess ||
+        cudaMallocHost((void **)&c->h_done, 2 * sizeof(int)) != cudaSuccess ||
+        cudaMallocHost((void **)&c->h_results, (kMaxShifts + 1) * sizeof(double)) != cudaSuccess)
+        return cleanup(QCD_ENOMEM, "qcd_create: pinned allocation failed");
+    if (cudaEventCreateWithFlags(&c->ev[0], cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev[1], cudaEventDisableTiming) != cudaSuccess ||
+        cudaMemset(c->st, 0, sizeof(CgState)) != cudaSuccess)
+        return cleanup(QCD_ECUDA, "qcd_create: event/memset failed");
+    *out = c;
+    return QCD_OK;
+}
+
+qcd_status qcd_destroy(qcd_ctx *c)
+{
+    if (!c) return QCD_OK;
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->W); cudaFree(c->tmp); cudaFree(c->q); cudaFree(c->r); cudaFree(c->p);
+    cudaFree(c->xws); cudaFree(c->partial); cudaFree(c->st); cudaFree(c->results);
+    cudaFree(c->stage_links); cudaFree(c->stage_vec); cudaFree(c->hv_a); cudaFree(c->hv_b);
+    cudaFree(c->hv_y);
+    if (c->h_state) cudaFreeHost(c->h_state);
+    if (c->h_done) cudaFreeHost(c->h_done);
+    if (c->h_results) cudaFreeHost(c->h_results);
+    for (auto &e : c->ev) if (e) cudaEventDestroy(e);
+    delete c;
+    return QCD_OK;
+}
+
+qcd_status qcd_set_mass(qcd_ctx *c, double mass)
+{
+    if (!c) return QCD_EINVAL;
+    if (!(mass == mass)) return fail(c, QCD_EINVAL, "qcd_set_mass: mass is NaN");
+    c->mass = mass;
+    return QCD_OK;
+}
+
+qcd_status qcd_set_stream(qcd_ctx *c, void *cuda_stream)
+{
+    if (!c) return QCD_EINVAL;
+    c->stream = (cudaStream_t)cuda_stream;
+    return QCD_OK;
+}
+
+long qcd_vector_doubles(const qcd_ctx *c) { return c ? 2 * c->n2 : 0; }
+long qcd_launch_count(const qcd_ctx *c) { return c ? c->launches : 0; }
+const char *qcd_last_error(const qcd_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
+
+qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
+{
+    if (!c) return QCD_EINVAL;
+    if (!d_links) return fail(c, QCD_EINVAL, "qcd_load_gauge: NULL links");
+    c->launches += launch_ingest_links(c->g, d_links, c->W, c->stream);
+    qcd_status s = check_launch(c, "qcd_load_gauge");
+    if (s == QCD_OK) c->gauge_loaded = true;
+    return s;
+}
+
+qcd_status qcd_load_gauge_host(qcd_ctx *c, const double *h_links)
+{
+    if (!c) return QCD_EINVAL;
+    if (!h_links) return fail(c, QCD_EINVAL, "qcd_load_gauge_host: NULL links");
+    const size_t bytes = (size_t)144 * c->g.Vh * sizeof(double);   // 72 V doubles
+    if (!c->stage_links) QCD_CUDA(c, cudaMalloc((void **)&c->stage_links, bytes));
+    QCD_CUDA(c, cudaMemcpyAsync(c->stage_links, h_links, bytes, cudaMemcpyHostToDevice, c->stream));
+    qcd_status s = qcd_load_gauge(c, c->stage_links);
+    if (s != QCD_OK) return s;
+    QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return QCD_OK;
+}
+
+qcd_status qcd_pack(qcd_ctx *c, int parity, const double *d_canon, double *d_internal)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(parity) || !d_canon || !d_internal || d_canon == d_internal)
+        return fail(c, QCD_EINVAL, "qcd_pack: bad argument");
+    c->launches += launch_pack(c->g, d_canon, (double2 *)d_internal, c->stream);
+    return check_launch(c, "qcd_pack");
+}
+
+qcd_status qcd_unpack(qcd_ctx *c, int parity, const double *d_internal, double *d_canon)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(parity) || !d_canon || !d_internal || d_canon == d_internal)
+        return fail(c, QCD_EINVAL, "qcd_unpack: bad argument");
+    c->launches += launch_unpack(c->g, (const double2 *)d_internal, d_canon, c->stream);
+    return check_launch(c, "qcd_unpack");
+}
+
+qcd_status qcd_dslash(qcd_ctx *c, int out_parity, const double *d_in, double *d_out)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(out_parity) || !d_in || !d_out || d_in == d_out)
+        return fail(c, QCD_EINVAL, "qcd_dslash: bad argument");
+    if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_dslash: no gauge field loaded");
+    run_dslash(c, out_parity, (const double2 *)d_in, (double2 *)d_out, nullptr, 0.0, false, 0, false);
+    return check_launch(c, "qcd_dslash");
+}
+
+qcd_status qcd_mdagm(qcd_ctx *c, int parity, const double *d_in, double *d_out)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(parity) || !d_in || !d_out || d_in == d_out)
+        return fail(c, QCD_EINVAL, "qcd_mdagm: bad argument");
+    if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_mdagm: no gauge field loaded");
+    const double2 *in = (const double2 *)d_in;
+    run_dslash(c, 1 - parity, in, c->tmp, nullptr, 0.0, false, 0, false);
+    run_dslash(c, parity, c->tmp, (double2 *)d_out, in, c->mass * c->mass, false, 0, false);
+    return check_launch(c, "qcd_mdagm");
+}
+
+qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshift,
+                             const double *shifts, const double *residues, double tol,
+                             int max_iter, double *d_x, double *d_y, int *iterations,
+                             double *true_res)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(parity) || !d_b || !shifts || !residues || !iterations || !true_res)
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg: NULL argument or bad parity");
+    if (nshift < 1 || nshift > kMaxShifts)
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg: nshift must be in [1, QCD_MAX_SHIFTS]");
+    if (!(tol > 0.0) || max_iter < 1)
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg: tol must be > 0 and max_iter >= 1");
+    for (int k = 0; k < nshift; ++k)
+        if (!(shifts[k] >= 0.0)) return fail(c, QCD_EINVAL, "qcd_multishift_cg: shifts must be >= 0");
+    if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_multishift_cg: no gauge field loaded");
+    qcd_status s = ensure_cg_workspace(c, nshift, d_x == nullptr);
+    if (s != QCD_OK) return s;
+
+    const long n2 = c->n2;
+    cudaStream_t st = c->stream;
+    const double2 *b = (const double2 *)d_b;
+    double2 *x = d_x ? (double2 *)d_x : c->xws;
+
+    // base system = smallest shift (C12): sort, remember the caller's order
+    std::vector<int> order(nshift);
+    for (int k = 0; k < nshift; ++k) order[k] = k;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int bb) { return shifts[a] < shifts[bb]; });
+
+    CgState &h = *c->h_state;
+    QCD_CUDA(c, cudaStreamSynchronize(st));   // h_state may still be in flight from a previous solve
+    std::memset(&h, 0, sizeof h);
+    h.alpha_old = 1.0; h.beta_old = 0.0;
+    h.tol = tol; h.freeze = 0.1;
+    h.nshift = nshift; h.max_iter = max_iter;
+    std::vector<long long> xoff_caller(nshift);
+    for (int k = 0; k < nshift; ++k) {
+        h.sigma[k] = shifts[order[k]];
+        h.zeta[k] = h.zeta_old[k] = h.zeta_new[k] = 1.0;
+        h.active[k] = 1;
+        h.xoff[k] = (long long)(d_x ? order[k] : k) * n2;
+        xoff_caller[order[k]] = h.xoff[k];
+    }
+    h.sigma0 = h.sigma[0];
+    QCD_CUDA(c, cudaMemcpyAsync(c->st, &h, sizeof h, cudaMemcpyHostToDevice, st));
+    QCD_CUDA(c, cudaMemsetAsync(x, 0, (size_t)n2 * nshift * sizeof(double2), st));
+    c->launches += launch_cg_init(n2, b, c->r, c->p, n2, nshift, c->partial, c->st, st);
+
+    // iteration loop: enqueue only
+    const int batch = 16;
+    int enq = 0, cur = 0;
+    bool pending = false, finished = false;
+    c->h_done[0] = c->h_done[1] = 0;
+    while (!finished && enq < max_iter) {
+        const int nb = std::min(batch, max_iter - enq);
+        for (int i = 0; i < nb; ++i) {
+            // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
+            run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
+            run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
+            c->launches += launch_cg_update_r(n2, c->r, c->q, c->partial, c->st, st);
+            c->launches += launch_cg_update_shifts(n2, c->r, x, c->p, n2, c->st, st);
+        }
+        enq += nb;
+        if (pending) {
+            QCD_CUDA(c, cudaEventSynchronize(c->ev[1 - cur]));
+            if (c->h_done[1 - cur]) finished = true;
+        }
+        QCD_CUDA(c, cudaMemcpyAsync(&c->h_done[cur], &c->st->done, sizeof(int), cudaMemcpyDeviceToHost, st));
+        QCD_CUDA(c, cudaEventRecord(c->ev[cur], st));
+        pending = true;
+        cur = 1 - cur;
+    }
+
+    // finish (a6): true residuals recomputed from x_k, y = sum_k c_k x_k
+    for (int k = 0; k < nshift; ++k) {
+        const double2 *xk = x + h.xoff[k];
+        run_dslash(c, 1 - parity, xk, c->tmp, nullptr, 0.0, false, 0, false);
+        run_dslash(c, parity, c->tmp, c->q, xk, c->mass * c->mass, false, 0, false);
+        c->launches += launch_residual_norm(n2, b, c->q, xk, h.sigma[k], c->partial, c->st,
+                                            c->results + order[k], st);
+    }
+    if (d_y)
+        c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, (double2 *)d_y, st);
+    s = check_launch(c, "qcd_multishift_cg");
+    if (s != QCD_OK) return s;
+    QCD_CUDA(c, cudaMemcpyAsync(c->h_results, c->results, nshift * sizeof(double), cudaMemcpyDeviceToHost, st));
+    QCD_CUDA(c, cudaMemcpyAsync(&h, c->st, sizeof h, cudaMemcpyDeviceToHost, st));
+    QCD_CUDA(c, cudaStreamSynchronize(st));
+
+    *iterations = h.iter;
+    const double rho_b = h.rho_b;
+    for (int k = 0; k < nshift; ++k)
+        true_res[k] = rho_b > 0.0 ? std::sqrt(c->h_results[k] / rho_b) : 0.0;
+    const bool converged = rho_b == 0.0 || std::sqrt(h.rho / rho_b) <= tol;
+    if (!converged) return fail(c, QCD_ENOTCONV, "qcd_multishift_cg: max_iter reached");
+    return QCD_OK;
+}
+
+qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, double *h_out)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(out_parity) || !h_in || !h_out)
+        return fail(c, QCD_EINVAL, "qcd_dslash_host: bad argument");
+    qcd_status s = ensure_host_staging(c);
+    if (s != QCD_OK) return s;
+    QCD_CUDA(c, cudaMemcpyAsync(c->stage_vec, h_in, c->vec_bytes, cudaMemcpyHostToDevice, c->stream));
+    if ((s = qcd_pack(c, 1 - out_parity, c->stage_vec, (double *)c->hv_a)) != QCD_OK) return s;
+    if ((s = qcd_dslash(c, out_parity, (double *)c->hv_a, (double *)c->hv_b)) != QCD_OK) return s;
+    if ((s = qcd_unpack(c, out_parity, (double *)c->hv_b, c->stage_vec)) != QCD_OK) return s;
+    QCD_CUDA(c, cudaMemcpyAsync(h_out, c->stage_vec, c->vec_bytes, cudaMemcpyDeviceToHost, c->stream));
+    QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return QCD_OK;
+}
+
+qcd_status qcd_mdagm_host(qcd_ctx *c, int parity, const double *h_in, double *h_out)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(parity) || !h_in || !h_out)
+        return fail(c, QCD_EINVAL, "qcd_mdagm_host: bad argument");
+    qcd_status s = ensure_host_staging(c);
+    if (s != QCD_OK) return s;
+    QCD_CUDA(c, cudaMemcpyAsync(c->stage_vec, h_in, c->vec_bytes, cudaMemcpyHostToDevice, c->stream));
+    if ((s = qcd_pack(c, parity, c->stage_vec, (double *)c->hv_a)) != QCD_OK) return s;
+    if ((s = qcd_mdagm(c, parity, (double *)c->hv_a, (double *)c->hv_b)) != QCD_OK) return s;
+    if ((s = qcd_unpack(c, parity, (double *)c->hv_b, c->stage_vec)) != QCD_OK) return s;
+    QCD_CUDA(c, cudaMemcpyAsync(h_out, c->stage_vec, c->vec_bytes, cudaMemcpyDeviceToHost, c->stream));
+    QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return QCD_OK;
+}
+
+qcd_status qcd_multishift_cg_host(qcd_ctx *c, int parity, const double *h_b, int nshift,
+                                  const double *shifts, const double *residues, double tol,
+                                  int max_iter, double *h_x, double *h_y, int *iterations,
+                                  double *true_res)
+{
+    if (!c) return QCD_EINVAL;
+    if (!h_b) return fail(c, QCD_EINVAL, "qcd_multishift_cg_host: NULL source");
+    if (nshift < 1 || nshift > kMaxShifts)
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg_host: nshift must be in [1, QCD_MAX_SHIFTS]");
+    qcd_status s = ensure_host_staging(c);
+    if (s != QCD_OK) return s;
+    if ((s = ensure_cg_workspace(c, nshift, true)) != QCD_OK) return s;
+    if (!c->hv_y) QCD_CUDA(c, dev_alloc(&c->hv_y, (size_t)c->n2));
+    QCD_CUDA(c, cudaMemcpyAsync(c->stage_vec, h_b, c->vec_bytes, cudaMemcpyHostToDevice, c->stream));
+    if ((s = qcd_pack(c, parity, c->stage_vec, (double *)c->hv_a)) != QCD_OK) return s;
+    qcd_status solve = qcd_multishift_cg(c, parity, (double *)c->hv_a, nshift, shifts, residues, tol,
+                                         max_iter, nullptr, (double *)c->hv_y, iterations, true_res);
+    if (solve != QCD_OK && solve != QCD_ENOTCONV) return solve;
+    if (h_x) {
+        // workspace x is in sorted-shift order; return it in the caller's order
+        std::vector<int> order(nshift);
+        for (int k = 0; k < nshift; ++k) order[k] = k;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int bb) { return shifts[a] < shifts[bb]; });
+        for (int k = 0; k < nshift; ++k) {
+            if ((s = qcd_unpack(c, parity, (double *)(c->xws + (long)k * c->n2), c->stage_vec)) != QCD_OK) return s;
+            QCD_CUDA(c, cudaMemcpyAsync(h_x + (size_t)order[k] * 2 * c->n2, c->stage_vec, c->vec_bytes,
+                                        cudaMemcpyDeviceToHost, c->stream));
+        }
+    }
+    if (h_y) {
+        if ((s = qcd_unpack(c, parity, (double *)c->hv_y, c->stage_vec)) != QCD_OK) return s;
+        QCD_CUDA(c, cudaMemcpyAsync(h_y, c->stage_vec, c->vec_bytes, cudaMemcpyDeviceToHost, c->stream));
+    }
+    QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+    return solve;
+}
+
+}  // extern "C"

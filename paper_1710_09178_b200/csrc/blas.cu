@@ -1,0 +1,189 @@
+// blas.cu -- a5/a6 of SURVEY 8(a): fused BLAS-1 of the multishift CG.  Hand loops instead of BLAS
+// calls, reductions with an explicit reduction variable (the paper's own finding), and
+// light loops merged into heavier ones: the r-update carries the norm, the shift
+// update streams x_k and p_k of every active shift in one pass over r ("the heaviest kernel which
+// updates three large arrays").  All coefficients are read from the device-resident
+// CgState; nothing returns to the host inside an iteration.
+#include "cg_scalars.cuh"
+#include "reduce.cuh"
+
+namespace qcd {
+
+namespace {
+
+constexpr int kBlock = 256;
+constexpr int kMaxBlocks = 148 * 8;   // grid-stride above this: a multiple of the SM count
+
+// r = b ; p_k = b (all k) ; rho = rho_b = <b,b> ; x_k are zeroed by a memset
+__global__ void __launch_bounds__(kBlock)
+cg_init_kernel(long n2, const double2 *__restrict__ b, double2 *__restrict__ r,
+               double2 *__restrict__ p, long pstride, int nshift, double *partial, CgState *st)
+{
+    double s = 0.0;
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        const double2 v = __ldg(b + i);
+        r[i] = v;
+        for (int k = 0; k < nshift; ++k) p[k * pstride + i] = v;
+        s += v.x * v.x + v.y * v.y;
+    }
+    double total;
+    if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total)) {
+        if (threadIdx.x == 0) {
+            st->rho = total;
+            st->rho_b = total;
+            if (total == 0.0) { st->done = 1; st->done_prev = 1; }   // b = 0: x_k = 0 is exact
+        }
+    }
+}
+
+// r -= alpha q ; rho' = <r,r> ; last block: beta, beta_k, zeta rotation, freezing, stop test
+__global__ void __launch_bounds__(kBlock)
+cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q, double *partial,
+                   CgState *st)
+{
+    if (st->done) {                       // dead iteration after convergence
+        if (blockIdx.x == 0 && threadIdx.x == 0) st->done_prev = 1;
+        return;
+    }
+    const double alpha = st->alpha;
+    double s = 0.0;
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        double2 rv = r[i];
+        const double2 qv = __ldg(q + i);
+        rv.x = fma(-alpha, qv.x, rv.x);
+        rv.y = fma(-alpha, qv.y, rv.y);
+        r[i] = rv;
+        s += rv.x * rv.x + rv.y * rv.y;
+    }
+    double total;
+    if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total)) cg_step_beta(st, total);
+}
+
+// for every shift k updated this iteration:  x_k += alpha_k p_k ;  p_k = zeta_k^new r + beta_k p_k
+__global__ void __launch_bounds__(kBlock)
+cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restrict__ x,
+                        double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
+{
+    if (st->done_prev) return;
+    __shared__ double s_a[kMaxShifts], s_z[kMaxShifts], s_b[kMaxShifts];
+    __shared__ long long s_x[kMaxShifts], s_p[kMaxShifts];
+    const int nl = st->nlist;
+    if (threadIdx.x < nl) {
+        const int k = st->list[threadIdx.x];
+        s_a[threadIdx.x] = st->coef_a[k];
+        s_z[threadIdx.x] = st->coef_z[k];
+        s_b[threadIdx.x] = st->coef_b[k];
+        s_x[threadIdx.x] = st->xoff[k];
+        s_p[threadIdx.x] = (long long)k * pstride;
+    }
+    __syncthreads();
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        const double2 rv = __ldg(r + i);
+#pragma unroll 4
+        for (int j = 0; j < nl; ++j) {
+            double2 *xp = x + s_x[j] + i;
+            double2 *pp = p + s_p[j] + i;
+            double2 xv = *xp;
+            double2 pv = *pp;
+            const double a = s_a[j], z = s_z[j], bb = s_b[j];
+            xv.x = fma(a, pv.x, xv.x);
+            xv.y = fma(a, pv.y, xv.y);
+            pv.x = fma(bb, pv.x, z * rv.x);
+            pv.y = fma(bb, pv.y, z * rv.y);
+            *xp = xv;
+            *pp = pv;
+        }
+    }
+}
+
+// *result = || b - (q + sigma x) ||^2   (q == nullptr: *result = ||b||^2)
+__global__ void __launch_bounds__(kBlock)
+residual_norm_kernel(long n2, const double2 *__restrict__ b, const double2 *__restrict__ q,
+                     const double2 *__restrict__ x, double sigma, double *partial, CgState *st,
+                     double *result)
+{
+    double s = 0.0;
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        double2 d = __ldg(b + i);
+        if (q != nullptr) {
+            const double2 qv = __ldg(q + i), xv = __ldg(x + i);
+            d.x -= fma(sigma, xv.x, qv.x);
+            d.y -= fma(sigma, xv.y, qv.y);
+        }
+        s += d.x * d.x + d.y * d.y;
+    }
+    double total;
+    if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total))
+        if (threadIdx.x == 0) *result = total;
+}
+
+struct CombineArgs {
+    long long xoff[kMaxShifts];
+    double c[kMaxShifts];
+    int n;
+};
+
+// y = sum_k c_k x_k   (eq. 8 without c_0)
+__global__ void __launch_bounds__(kBlock)
+combine_kernel(long n2, const double2 *__restrict__ x, const CombineArgs a, double2 *__restrict__ y)
+{
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        double2 s = make_double2(0.0, 0.0);
+#pragma unroll 4
+        for (int k = 0; k < a.n; ++k) {
+            const double2 v = __ldg(x + a.xoff[k] + i);
+            s.x = fma(a.c[k], v.x, s.x);
+            s.y = fma(a.c[k], v.y, s.y);
+        }
+        y[i] = s;
+    }
+}
+
+}  // namespace
+
+int blas_grid_blocks(long n2)
+{
+    long b = (n2 + kBlock - 1) / kBlock;
+    return (int)(b < kMaxBlocks ? (b > 0 ? b : 1) : kMaxBlocks);
+}
+
+int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
+                   double *partial, CgState *st, cudaStream_t s)
+{
+    cg_init_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, b, r, p, pstride, nshift, partial, st);
+    return 1;
+}
+
+int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
+                       cudaStream_t s)
+{
+    cg_update_r_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, r, q, partial, st);
+    return 1;
+}
+
+int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
+                            CgState *st, cudaStream_t s)
+{
+    cg_update_shifts_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, r, x, p, pstride, st);
+    return 1;
+}
+
+int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
+                         double *partial, CgState *st, double *result, cudaStream_t s)
+{
+    residual_norm_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, b, q, x, sigma, partial, st,
+                                                                 result);
+    return 1;
+}
+
+int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
+                   int nshift, double2 *y, cudaStream_t s)
+{
+    CombineArgs a;
+    a.n = nshift;
+    for (int k = 0; k < nshift; ++k) { a.xoff[k] = xoff_host[k]; a.c[k] = residues[k]; }
+    combine_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, x, a, y);
+    return 1;
+}
+
+}  // namespace qcd

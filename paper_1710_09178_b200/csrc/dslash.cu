@@ -1,0 +1,130 @@
+// dslash.cu -- a2/a3/a4 of SURVEY 8(a): the even-odd staggered Dirac operator
+//   out(x) = sum_mu [ W_mu(x) in(x+mu) - W_mu(x-mu)^dag in(x-mu) ],  x of parity out_parity
+// (PAPER.md:106 with 1/2, eta and the t-seam sign folded into W, see layout.cu), optionally fused
+// with out = coeff*src - (.) (the m^2 term of M^dag M) and with the partial sums of
+// Re<src,out> whose last block runs the CG alpha/zeta step.
+//
+// HBM-bound stencil: 8 links (1152 B) + 48 B out per site, neighbour vectors mostly from L2/L1;
+// 570 flop / 1248 B = 0.46 flop/B, so no tensor cores (BASELINE.json north_star).  One thread per
+// output site, site-fastest planes: every load/store of a warp is a contiguous run of 16-byte
+// elements (LDG.128/STG.128).
+#include "cg_scalars.cuh"
+#include "reduce.cuh"
+
+namespace qcd {
+
+namespace {
+
+constexpr int kBlock = 128;
+
+// acc += w * v
+__device__ __forceinline__ void cmad(double2 &acc, const double2 w, const double2 v)
+{
+    acc.x = fma(w.x, v.x, acc.x);
+    acc.x = fma(-w.y, v.y, acc.x);
+    acc.y = fma(w.x, v.y, acc.y);
+    acc.y = fma(w.y, v.x, acc.y);
+}
+// acc -= conj(w) * v
+__device__ __forceinline__ void cmsub_conj(double2 &acc, const double2 w, const double2 v)
+{
+    acc.x = fma(-w.x, v.x, acc.x);
+    acc.x = fma(-w.y, v.y, acc.x);
+    acc.y = fma(-w.x, v.y, acc.y);
+    acc.y = fma(w.y, v.x, acc.y);
+}
+
+template <bool XPAY, bool DOT>
+__global__ void __launch_bounds__(kBlock)
+dslash_kernel(const Geom g, const DslashParams p)
+{
+    if (p.st != nullptr && p.st->done) return;   // CG already converged: dead iteration
+    const int Vh = g.Vh;
+    const uint32_t h = blockIdx.x * kBlock + threadIdx.x;
+    const bool valid = h < (uint32_t)Vh;
+    double dot = 0.0;
+    if (valid) {
+        uint32_t q, xh, y, z, t;
+        g.dxh.divmod(h, q, xh);
+        g.dy.divmod(q, q, y);
+        g.dz.divmod(q, t, z);
+        const int par = p.out_parity;
+        const int r = (y + z + t + par) & 1;      // x = 2*xh + r
+        // half indices of the 8 neighbours (all of the opposite parity)
+        int hp[4], hm[4];
+        {
+            const int xh_p = r ? ((int)xh + 1 == g.Nxh ? 0 : (int)xh + 1) : (int)xh;
+            const int xh_m = r ? (int)xh : (xh == 0 ? g.Nxh - 1 : (int)xh - 1);
+            hp[0] = (int)h - (int)xh + xh_p;
+            hm[0] = (int)h - (int)xh + xh_m;
+            hp[1] = (int)h + ((int)y + 1 == g.Ny ? -(g.Ny - 1) * g.sy : g.sy);
+            hm[1] = (int)h + (y == 0 ? (g.Ny - 1) * g.sy : -g.sy);
+            hp[2] = (int)h + ((int)z + 1 == g.Nz ? -(g.Nz - 1) * g.sz : g.sz);
+            hm[2] = (int)h + (z == 0 ? (g.Nz - 1) * g.sz : -g.sz);
+            hp[3] = (int)h + ((int)t + 1 == g.Nt ? -(g.Nt - 1) * g.st : g.st);
+            hm[3] = (int)h + (t == 0 ? (g.Nt - 1) * g.st : -g.st);
+        }
+        const double2 *__restrict__ in = p.in;
+        double2 acc[3];
+        acc[0] = acc[1] = acc[2] = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            {   // forward hop: + W_mu(x) in(x+mu), link based at x (parity par)
+                const double2 *__restrict__ w = p.W + ((long)(par * 4 + mu) * 9) * Vh + h;
+                double2 v[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hp[mu]);
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b) cmad(acc[a], __ldg(w + (long)(a * 3 + b) * Vh), v[b]);
+            }
+            {   // backward hop: - W_mu(x-mu)^dag in(x-mu), link based at x-mu (parity 1-par)
+                const double2 *__restrict__ w = p.W + ((long)((1 - par) * 4 + mu) * 9) * Vh + hm[mu];
+                double2 v[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hm[mu]);
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+                        cmsub_conj(acc[a], __ldg(w + (long)(b * 3 + a) * Vh), v[b]);
+            }
+        }
+        if (XPAY) {
+            const double coeff = p.coeff_from_state ? p.mass2 + p.st->sigma0 : p.coeff;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const double2 s = __ldg(p.src + (long)c * Vh + h);
+                acc[c].x = fma(coeff, s.x, -acc[c].x);
+                acc[c].y = fma(coeff, s.y, -acc[c].y);
+                if (DOT) dot += s.x * acc[c].x + s.y * acc[c].y;
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) p.out[(long)c * Vh + h] = acc[c];
+    }
+    if (DOT) {
+        double total;
+        if (grid_sum_last_block<kBlock>(dot, p.partial, &p.st->counter, total))
+            cg_step_alpha(p.st, total);
+    }
+}
+
+}  // namespace
+
+int dslash_grid_blocks(const Geom &g) { return (g.Vh + kBlock - 1) / kBlock; }
+
+int launch_dslash(const Geom &g, const DslashParams &p, cudaStream_t s)
+{
+    const int blocks = dslash_grid_blocks(g);
+    if (p.src == nullptr)
+        dslash_kernel<false, false><<<blocks, kBlock, 0, s>>>(g, p);
+    else if (p.dot_mode == 0)
+        dslash_kernel<true, false><<<blocks, kBlock, 0, s>>>(g, p);
+    else
+        dslash_kernel<true, true><<<blocks, kBlock, 0, s>>>(g, p);
+    return 1;
+}
+
+}  // namespace qcd

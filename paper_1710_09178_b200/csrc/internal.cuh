@@ -1,0 +1,99 @@
+// internal.cuh -- shared declarations of the CUDA library (not part of the ABI).
+//
+// Internal HBM layout:
+//   parity vector  double2 v[3][Vh]               colour-major planes, site-fastest ("ap(V,3)")
+//   links          double2 W[2][4][9][Vh]         [parity of the link's base site][mu][row*3+col][h]
+//                  W_mu(x) = 1/2 eta_mu(x) s+_mu(x) U_mu(x)   (phases absorbed)
+//   half index     h = ((t*Nz + z)*Ny + y)*(Nx/2) + x/2   == canonical address l >> 1
+// so that (D psi)(x) = sum_mu [ W_mu(x) psi(x+mu) - W_mu(x-mu)^dag psi(x-mu) ].
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/qcd.h"
+
+namespace qcd {
+
+constexpr int kMaxShifts = QCD_MAX_SHIFTS;
+
+// n / d for 0 <= n < 2^31 with one mulhi (d fixed at context creation).
+struct FastDiv {
+    uint32_t d, magic, shift;
+    __host__ void init(uint32_t div)
+    {
+        d = div;
+        shift = 0;
+        while ((1u << shift) < div) ++shift;
+        magic = (uint32_t)(((uint64_t(1) << 32) * ((uint64_t(1) << shift) - div)) / div + 1);
+    }
+    __device__ __forceinline__ void divmod(uint32_t n, uint32_t &q, uint32_t &r) const
+    {
+        q = (__umulhi(n, magic) + n) >> shift;
+        r = n - q * d;
+    }
+};
+
+struct Geom {
+    int Nx, Ny, Nz, Nt, Nxh;
+    int Vh;          // sites of one parity
+    int sy, sz, st;  // half-index strides of +y, +z, +t
+    FastDiv dxh, dy, dz;
+};
+
+// Device-resident scalars of the multishift CG; no host round trip per iteration.
+struct CgState {
+    double rho, rho_b, pAp, alpha, beta, alpha_old, beta_old;
+    double tol, freeze, sigma0;
+    double sigma[kMaxShifts];     // sorted ascending, sigma[0] = base
+    double zeta[kMaxShifts], zeta_old[kMaxShifts], zeta_new[kMaxShifts];
+    double coef_a[kMaxShifts], coef_z[kMaxShifts], coef_b[kMaxShifts];  // x_k += a p_k ; p_k = z r + b p_k
+    long long xoff[kMaxShifts];   // element (double2) offset of x_k in the x buffer
+    int list[kMaxShifts];         // compacted indices of the shifts updated this iteration
+    int nlist;
+    int active[kMaxShifts];
+    int nshift, iter, max_iter;
+    int done;                     // set by the r-update of the converging iteration
+    int done_prev;                // set one (dead) iteration later: gates the shift update
+    unsigned counter;             // last-block-done ticket
+    double scratch;               // generic reduction result (norms for true residuals)
+};
+
+// ---- launchers (each enqueues on `s` and returns the number of kernels launched) ----
+
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, cudaStream_t s);
+int launch_pack(const Geom &g, const double *canon, double2 *internal, cudaStream_t s);
+int launch_unpack(const Geom &g, const double2 *internal, double *canon, cudaStream_t s);
+
+struct DslashParams {
+    const double2 *W;
+    const double2 *in;
+    double2 *out;
+    int out_parity;
+    // optional fused epilogue: out = coeff * src - D in     (src on out_parity); src == nullptr: out = D in
+    const double2 *src;
+    double coeff;              // used when coeff_from_state == 0
+    int coeff_from_state;      // 1: coeff = mass2 + st->sigma0 read on device
+    double mass2;
+    // optional fused <src,out> with the CG alpha/zeta step in the last block
+    int dot_mode;              // 0 none, 1 CG (pAp -> alpha, zeta_new, coef_a)
+    double *partial;
+    CgState *st;               // also the early-exit flag when non-null
+};
+int launch_dslash(const Geom &g, const DslashParams &p, cudaStream_t s);
+int dslash_grid_blocks(const Geom &g);
+
+// BLAS-1 (n2 = 3*Vh double2 elements per vector)
+int blas_grid_blocks(long n2);
+int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
+                   double *partial, CgState *st, cudaStream_t s);
+int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
+                       cudaStream_t s);
+int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
+                            CgState *st, cudaStream_t s);
+// scratch = || b - (q + sigma x) ||^2   and  scratch = ||b||^2
+int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
+                         double *partial, CgState *st, double *result, cudaStream_t s);
+int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
+                   int nshift, double2 *y, cudaStream_t s);
+
+}  // namespace qcd

@@ -1,0 +1,89 @@
+// layout.cu -- a1 of SURVEY 8(a): canonical (lexicographic AoS) <-> internal (parity-split SoA).
+//
+// Links: W_mu(x) = 1/2 eta_mu(x) s+_mu(x) U_mu(x).  The paper absorbs the staggered phases into the
+// stored links; here the 1/2 of the M = m + D normalisation and the
+// antiperiodic sign of the t-seam hop (C5) are folded in as well.  Because eta_mu does not depend on
+// x_mu, and s-_mu(x) = s+_mu(x - mu), the backward hop at x needs exactly W_mu(x - mu)^dag.
+#include "internal.cuh"
+
+namespace qcd {
+
+namespace {
+
+constexpr int kBlock = 256;
+
+// one thread per (half index h, parity of the base site): 4 links each
+__global__ void __launch_bounds__(kBlock)
+ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__ W)
+{
+    const int Vh = g.Vh;
+    uint32_t tid = blockIdx.x * kBlock + threadIdx.x;
+    if (tid >= 2u * Vh) return;
+    int par = tid >= (uint32_t)Vh;
+    uint32_t h = tid - par * Vh;
+    uint32_t q, xh, y, z, t;
+    g.dxh.divmod(h, q, xh);
+    g.dy.divmod(q, q, y);
+    g.dz.divmod(q, t, z);
+    int x = 2 * xh + ((y + z + t + par) & 1);
+    long l = 2L * h + (x & 1);                      // canonical address: h = l >> 1
+    // eta_mu(x) = (-1)^(sum_{nu<mu} x_nu)
+    double eta[4] = {1.0, (x & 1) ? -1.0 : 1.0, ((x + y) & 1) ? -1.0 : 1.0,
+                     ((x + y + z) & 1) ? -1.0 : 1.0};
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        double f = 0.5 * eta[mu];
+        if (mu == 3 && t == (uint32_t)g.Nt - 1) f = -f;   // s+ across the t seam (C5)
+        const double2 *u = U + (l * 4 + mu) * 9;
+        double2 *w = W + ((long)(par * 4 + mu) * 9) * Vh + h;
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+            double2 v = u[c];
+            w[(long)c * Vh] = make_double2(f * v.x, f * v.y);
+        }
+    }
+}
+
+// canonical parity vector [j][3] (j == h) -> planes [3][Vh]
+__global__ void __launch_bounds__(kBlock)
+pack_kernel(int Vh, const double2 *__restrict__ canon, double2 *__restrict__ v)
+{
+    int h = blockIdx.x * kBlock + threadIdx.x;
+    if (h >= Vh) return;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) v[(long)c * Vh + h] = canon[3L * h + c];
+}
+
+__global__ void __launch_bounds__(kBlock)
+unpack_kernel(int Vh, const double2 *__restrict__ v, double2 *__restrict__ canon)
+{
+    int h = blockIdx.x * kBlock + threadIdx.x;
+    if (h >= Vh) return;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) canon[3L * h + c] = v[(long)c * Vh + h];
+}
+
+}  // namespace
+
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, cudaStream_t s)
+{
+    int blocks = (2 * g.Vh + kBlock - 1) / kBlock;
+    ingest_links_kernel<<<blocks, kBlock, 0, s>>>(g, (const double2 *)links_canon, W);
+    return 1;
+}
+
+int launch_pack(const Geom &g, const double *canon, double2 *internal, cudaStream_t s)
+{
+    int blocks = (g.Vh + kBlock - 1) / kBlock;
+    pack_kernel<<<blocks, kBlock, 0, s>>>(g.Vh, (const double2 *)canon, internal);
+    return 1;
+}
+
+int launch_unpack(const Geom &g, const double2 *internal, double *canon, cudaStream_t s)
+{
+    int blocks = (g.Vh + kBlock - 1) / kBlock;
+    unpack_kernel<<<blocks, kBlock, 0, s>>>(g.Vh, internal, (double2 *)canon);
+    return 1;
+}
+
+}  // namespace qcd

@@ -1,0 +1,60 @@
+// reduce.cuh -- deterministic grid-wide sum: warp shuffle -> block -> per-block partial ->
+// the last block to finish sums the partials in a fixed order ("warp-shuffle dot
+// and norm reductions", no second kernel, no host sync, bit-reproducible for a fixed grid).
+#pragma once
+#include "internal.cuh"
+
+namespace qcd {
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum over the block; result valid in every thread. BLOCK multiple of 32, <= 1024.
+template <int BLOCK>
+__device__ __forceinline__ double block_sum(double v)
+{
+    __shared__ double sm[32];
+    __shared__ double total;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    v = warp_sum(v);
+    __syncthreads();  // protects sm/total against a previous call
+    if (lane == 0) sm[wid] = v;
+    __syncthreads();
+    if (wid == 0) {
+        double t = lane < BLOCK / 32 ? sm[lane] : 0.0;
+        t = warp_sum(t);
+        if (lane == 0) total = t;
+    }
+    __syncthreads();
+    return total;
+}
+
+// Every block contributes v (already summed over its threads' work).  Returns true in ALL threads
+// of the one block that finishes last, with `total` = sum over all blocks in blockIdx order.
+template <int BLOCK>
+__device__ __forceinline__ bool grid_sum_last_block(double v, double *partial, unsigned *counter,
+                                                    double &total)
+{
+    __shared__ bool is_last;
+    double b = block_sum<BLOCK>(v);
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x] = b;
+        __threadfence();
+        unsigned ticket = atomicAdd(counter, 1u);
+        is_last = (ticket == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+    double t = 0.0;
+    for (unsigned i = threadIdx.x; i < gridDim.x; i += BLOCK) t += __ldcg(partial + i);
+    total = block_sum<BLOCK>(t);
+    if (threadIdx.x == 0) *counter = 0u;
+    return true;
+}
+
+}  // namespace qcd

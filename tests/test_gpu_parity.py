@@ -1,0 +1,329 @@
+"""GPU parity: the CUDA library (through its C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  Dslash / M^dag M   relative L2 error <= 1e-13
+  multishift CG      recomputed true residual <= 1.5 tol for every shift;
+                     ||x_k - x_k^oracle|| / ||x_k^oracle|| <= 1e-9 against the polished oracle (C16).
+"""
+import numpy as np
+import pytest
+
+import lattice_inputs as li
+import oracle
+from helpers import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_OP = 1e-13
+TOL_X = 1e-9
+E, O = 0, 1
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def q():
+    import paper_1710_09178_b200 as q
+    q.load_library()          # fails loudly if the extension is missing: no fallback
+    return q
+
+
+class Rig:
+    """One lattice: oracle + CUDA context fed the same canonical arrays."""
+
+    def __init__(self, torch, q, dims, mass, links):
+        self.torch, self.q = torch, q
+        self.dims, self.mass = dims, mass
+        self.lat = oracle.Lattice(dims, links)
+        self.ctx = q.Context(dims, mass)
+        self.d_links = torch.from_numpy(links).cuda()
+        self.ctx.load_gauge(self.d_links)
+        self.nh = self.lat.volume // 2
+
+    def to_internal(self, parity, canon: np.ndarray):
+        d_c = self.torch.from_numpy(np.ascontiguousarray(canon)).cuda().reshape(-1)
+        d_i = self.ctx.new_vector()
+        self.ctx.pack(parity, d_c, d_i)
+        return d_i
+
+    def to_canonical(self, parity, d_i) -> np.ndarray:
+        d_c = self.torch.empty(self.ctx.vector_doubles, dtype=self.torch.float64, device="cuda")
+        self.ctx.unpack(parity, d_i, d_c)
+        return d_c.cpu().numpy().reshape(self.nh, 3, 2)
+
+    def dslash(self, out_parity, v):
+        d_out = self.ctx.new_vector()
+        self.ctx.dslash(out_parity, self.to_internal(1 - out_parity, v), d_out)
+        return self.to_canonical(out_parity, d_out)
+
+    def mdagm(self, parity, v):
+        d_out = self.ctx.new_vector()
+        self.ctx.mdagm(parity, self.to_internal(parity, v), d_out)
+        return self.to_canonical(parity, d_out)
+
+    def solve(self, parity, b, shifts, residues, tol, max_iter=100000, own_x=True):
+        n = len(shifts)
+        d_x = self.ctx.new_vector(n) if own_x else None
+        d_y = self.ctx.new_vector()
+        st, it, tr = self.ctx.multishift_cg(parity, self.to_internal(parity, b), shifts, residues,
+                                            tol, max_iter, d_x, d_y)
+        x = None
+        if own_x:
+            x = np.stack([self.to_canonical(parity, d_x[k]) for k in range(n)])
+        return dict(status=st, iterations=it, true_res=tr, x=x, y=self.to_canonical(parity, d_y))
+
+
+def make_rig(torch, q, dims, kind, mass, seed, eps=0.3):
+    return Rig(torch, q, dims, mass, li.make_links(dims, kind, seed, eps))
+
+
+# ------------------------------------------------------------------ layout
+
+def test_pack_unpack_roundtrip_bit_exact(torch, q):
+    rig = make_rig(torch, q, (4, 6, 2, 8), "random", 0.1, 3)
+    v = li.make_source(rig.dims, 3, 0)
+    for par in (E, O):
+        assert np.array_equal(rig.to_canonical(par, rig.to_internal(par, v)), v)
+
+
+# ------------------------------------------------------------------ Dslash, M^dag M
+
+SHAPES = [
+    ((2, 2, 2, 2), "random"),          # extents of 2: x+mu == x-mu (C8)
+    ((4, 4, 4, 4), "random"),          # config 1
+    ((8, 8, 8, 4), "near_identity"),   # config 2
+    ((4, 4, 2, 6), "random"),
+    ((2, 4, 6, 2), "near_identity"),
+    ((6, 2, 4, 8), "random"),
+    ((12, 6, 10, 4), "random"),        # Vh = 1440: several blocks and a ragged tail
+    ((10, 14, 6, 6), "near_identity"), # Vh = 2520, non power-of-two strides
+]
+
+
+@pytest.mark.parametrize("dims,kind", SHAPES)
+def test_dslash_and_mdagm_match_oracle(torch, q, dims, kind):
+    rig = make_rig(torch, q, dims, kind, 0.07, seed=sum(dims))
+    ve = li.make_source(dims, 41, E)
+    vo = li.make_source(dims, 42, O)
+    assert rel_l2(rig.dslash(O, ve), rig.lat.dslash(O, ve)) <= TOL_OP    # D_oe
+    assert rel_l2(rig.dslash(E, vo), rig.lat.dslash(E, vo)) <= TOL_OP    # D_eo
+    assert rel_l2(rig.mdagm(E, ve), rig.lat.mdagm(0.07, E, ve)) <= TOL_OP
+    assert rel_l2(rig.mdagm(O, vo), rig.lat.mdagm(0.07, O, vo)) <= TOL_OP
+
+
+def test_dslash_free_field_eigenvalue_on_gpu(torch, q):
+    """Property that holds at any size: U = 1, plane wave restricted to the even sites is an
+    eigenvector of (M^dag M)_ee with eigenvalue m^2 + sum sin^2 p (north_star closed form)."""
+    dims, mass = (8, 4, 6, 4), 0.3
+    rig = Rig(torch, q, dims, mass, li.unit_links(dims))
+    from helpers import coords
+    xyzt = coords(dims)
+    n = (3, 1, 2, 1)
+    p = np.array([2 * np.pi * n[0] / dims[0], 2 * np.pi * n[1] / dims[1], 2 * np.pi * n[2] / dims[2],
+                  2 * np.pi * (n[3] + 0.5) / dims[3]])
+    psi = (np.exp(1j * xyzt @ p)[:, None] * np.array([1.0, 2j, -0.5])[None, :])[li.site_parity(dims) == 0]
+    v = np.stack([psi.real, psi.imag], axis=-1)
+    out = rig.mdagm(E, v)
+    assert rel_l2(out, (mass ** 2 + (np.sin(p) ** 2).sum()) * v) < 1e-13
+
+
+def test_set_mass_changes_mdagm(torch, q):
+    rig = make_rig(torch, q, (4, 4, 4, 4), "random", 0.1, 1)
+    v = li.make_source(rig.dims, 1, E)
+    rig.ctx.set_mass(0.25)
+    assert rel_l2(rig.mdagm(E, v), rig.lat.mdagm(0.25, E, v)) <= TOL_OP
+
+
+# ------------------------------------------------------------------ multishift CG
+
+def check_solve(rig, cfg, b, shifts, res, out, exact=None):
+    assert out["status"] == 0
+    assert np.isfinite(out["true_res"]).all()
+    assert (out["true_res"] <= 1.5 * cfg.tol).all(), out["true_res"]
+    for k, s in enumerate(shifts):
+        # the library's own true residual agrees with one recomputed by the ORACLE's operator
+        xk = out["x"][k]
+        r = b - (rig.lat.mdagm(cfg.mass, cfg.parity, xk) + s * xk)
+        tr = np.linalg.norm(r) / np.linalg.norm(b)
+        assert abs(tr - out["true_res"][k]) <= 1e-3 * tr + 1e-15
+        if exact is not None:
+            assert rel_l2(xk, exact["x"][k]) <= TOL_X, (k, rel_l2(xk, exact["x"][k]))
+    y_from_x = np.tensordot(res, out["x"], axes=(0, 0))
+    assert rel_l2(out["y"], y_from_x) <= 1e-14
+    if exact is not None:
+        assert rel_l2(out["y"], exact["y"]) <= TOL_X
+
+
+@pytest.mark.parametrize("number", [1, 2])
+def test_multishift_cg_configs_1_2(torch, q, number):
+    cfg, links, b, shifts, res = li.make_config_inputs(number)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    out = rig.solve(cfg.parity, b, shifts, res, cfg.tol)
+    exact = rig.lat.solve_exact(cfg.mass, cfg.parity, b, shifts, res, cfg.tol)
+    check_solve(rig, cfg, b, shifts, res, out, exact)
+    ref = rig.lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, want_x=False)
+    assert abs(out["iterations"] - ref["iterations"]) <= max(2, ref["iterations"] // 50)
+
+
+def test_multishift_cg_is_deterministic(torch, q):
+    cfg, links, b, shifts, res = li.make_config_inputs(2)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    o1 = rig.solve(cfg.parity, b, shifts, res, cfg.tol)
+    o2 = rig.solve(cfg.parity, b, shifts, res, cfg.tol)
+    assert o1["iterations"] == o2["iterations"]
+    assert np.array_equal(o1["x"], o2["x"]) and np.array_equal(o1["y"], o2["y"])
+
+
+def test_multishift_cg_odd_parity_unsorted_shifts_zero_shift(torch, q):
+    dims, mass = (4, 6, 4, 4), 0.08
+    rig = make_rig(torch, q, dims, "random", mass, 7)
+    b = li.make_source(dims, 7, O)
+    shifts = np.array([0.5, 0.0, 2.0, 1e-3, 0.02])
+    res = np.array([1.0, -2.0, 0.5, 3.0, 0.25])
+    out = rig.solve(O, b, shifts, res, 1e-11)
+    exact = rig.lat.solve_exact(mass, O, b, shifts, res, 1e-11)
+    assert out["status"] == 0 and (out["true_res"] <= 1.5e-11).all()
+    for k in range(len(shifts)):
+        assert rel_l2(out["x"][k], exact["x"][k]) <= TOL_X
+    assert rel_l2(out["y"], exact["y"]) <= TOL_X
+
+
+def test_multishift_cg_without_x_buffer_and_single_shift(torch, q):
+    cfg, links, b, shifts, res = li.make_config_inputs(1)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    with_x = rig.solve(E, b, shifts, res, cfg.tol)
+    no_x = rig.solve(E, b, shifts, res, cfg.tol, own_x=False)
+    assert np.array_equal(with_x["y"], no_x["y"]) and np.array_equal(with_x["true_res"], no_x["true_res"])
+    one = rig.solve(E, b, shifts[:1], res[:1], cfg.tol)
+    assert rel_l2(one["x"][0], with_x["x"][0]) <= 1e-9
+
+
+def test_freezing_light_mass_16_shifts(torch, q):
+    """C13 on the GPU: zeta_k of large shifts would underflow to 0/0 without freezing."""
+    dims, mass = (4, 4, 4, 4), 0.005
+    rig = make_rig(torch, q, dims, "random", mass, 5)
+    b = li.make_source(dims, 5, E)
+    shifts = np.logspace(-6, np.log10(4.0), 16)
+    out = rig.solve(E, b, shifts, np.ones(16), 1e-10)
+    assert out["status"] == 0 and out["iterations"] > 300
+    assert np.isfinite(out["x"]).all() and (out["true_res"] <= 1.5e-10).all()
+    exact = rig.lat.solve_exact(mass, E, b, shifts, np.ones(16), 1e-10)
+    for k in range(16):
+        assert rel_l2(out["x"][k], exact["x"][k]) <= TOL_X
+
+
+def test_max_iter_and_zero_source(torch, q):
+    cfg, links, b, shifts, res = li.make_config_inputs(1)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    out = rig.solve(E, b, shifts, res, cfg.tol, max_iter=7)
+    assert out["status"] == 4 and out["iterations"] == 7          # QCD_ENOTCONV, outputs still written
+    ref = rig.lat.multishift_cg(cfg.mass, E, b, shifts, res, cfg.tol, max_iter=7)
+    assert rel_l2(out["x"], ref["x"]) < 1e-12
+    assert np.allclose(out["true_res"], ref["true_res"], rtol=1e-9)
+    zero = rig.solve(E, np.zeros_like(b), shifts, res, cfg.tol)
+    assert zero["status"] == 0 and zero["iterations"] == 0 and not zero["x"].any() and not zero["y"].any()
+
+
+def test_error_codes(torch, q):
+    ctx = q.Context((4, 4, 4, 4), 0.1)
+    v, w = ctx.new_vector(), ctx.new_vector()
+    with pytest.raises(q.QcdError, match="QCD_ESTATE"):
+        ctx.dslash(E, v, w)
+    ctx.load_gauge(torch.from_numpy(li.make_links((4, 4, 4, 4), "random", 1)).cuda())
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        ctx.dslash(E, v, v)
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        ctx.dslash(2, v, w)
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        ctx.multishift_cg(E, v, [-1.0], [1.0], 1e-10, 10)
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        ctx.multishift_cg(E, v, [1.0], [1.0], 0.0, 10)
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        q.Context((4, 4, 3, 4), 0.1)
+
+
+def test_host_entry_points_equal_device_entry_points(torch, q):
+    cfg, links, b, shifts, res = li.make_config_inputs(2)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    ctx2 = q.Context(cfg.dims, cfg.mass)
+    ctx2.load_gauge_host(links)
+    out = np.empty_like(b)
+    ctx2.dslash_host(O, b, out)
+    assert np.array_equal(out, rig.dslash(O, b))
+    ctx2.mdagm_host(E, b, out)
+    assert np.array_equal(out, rig.mdagm(E, b))
+    hx = np.empty((len(shifts),) + b.shape)
+    hy = np.empty_like(b)
+    st, it, tr = ctx2.multishift_cg_host(E, b, shifts, res, cfg.tol, 10000, hx, hy)
+    dev = rig.solve(E, b, shifts, res, cfg.tol)
+    assert st == 0 and it == dev["iterations"]
+    assert np.array_equal(hx, dev["x"]) and np.array_equal(hy, dev["y"])
+    assert np.array_equal(tr, dev["true_res"])
+
+
+# ------------------------------------------------------------------ full-size configs 3, 4, 5
+
+@pytest.mark.slow
+def test_config3_full_size(torch, q):
+    """32^3 x 8, the configuration the metric is quoted on: operators element by element, solve
+    against the polished oracle."""
+    cfg, links, b, shifts, res = li.make_config_inputs(3)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    vo = li.make_source(cfg.dims, 43, O)
+    assert rel_l2(rig.dslash(O, b), rig.lat.dslash(O, b)) <= TOL_OP
+    assert rel_l2(rig.dslash(E, vo), rig.lat.dslash(E, vo)) <= TOL_OP
+    assert rel_l2(rig.mdagm(E, b), rig.lat.mdagm(cfg.mass, E, b)) <= TOL_OP
+    out = rig.solve(E, b, shifts, res, cfg.tol)
+    exact = rig.lat.solve_exact(cfg.mass, E, b, shifts, res, cfg.tol)
+    check_solve(rig, cfg, b, shifts, res, out, exact)
+
+
+def _sampled_shift_check(rig, cfg, b, shifts, out, ks):
+    """Where the full oracle solve is out of reach: compare sampled shifts against independent
+    single-shift oracle CGs run to the floor, the rest through the recomputed residual."""
+    for k in ks:
+        xs, _, tr, st = rig.lat.cg(cfg.mass, cfg.parity, shifts[k], b, 1e-14, max_iter=2000)
+        assert st == 0 and tr < 1e-13
+        assert rel_l2(out["x"][k], xs) <= TOL_X, (k, rel_l2(out["x"][k], xs))
+
+
+@pytest.mark.slow
+def test_config4_full_size(torch, q):
+    cfg, links, b, shifts, res = li.make_config_inputs(4)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    assert rel_l2(rig.dslash(O, b), rig.lat.dslash(O, b)) <= TOL_OP
+    assert rel_l2(rig.mdagm(E, b), rig.lat.mdagm(cfg.mass, E, b)) <= TOL_OP
+    out = rig.solve(E, b, shifts, res, cfg.tol)
+    assert out["status"] == 0 and (out["true_res"] <= 1.5 * cfg.tol).all(), out["true_res"]
+    for k in (0, 7, 15):      # residual recomputed with the oracle's operator
+        xk = out["x"][k]
+        r = b - (rig.lat.mdagm(cfg.mass, E, xk) + shifts[k] * xk)
+        tr = np.linalg.norm(r) / np.linalg.norm(b)
+        assert tr <= 1.5 * cfg.tol and abs(tr - out["true_res"][k]) <= 1e-2 * tr
+    assert rel_l2(out["y"], np.tensordot(res, out["x"], axes=(0, 0))) <= 1e-14
+    _sampled_shift_check(rig, cfg, b, shifts, out, ks=(13, 15))
+
+
+@pytest.mark.slow
+def test_config5_full_size(torch, q):
+    """64^3 x 16, random SU(3), m = 0.005: thousands of iterations; the full oracle solve would
+    take hours on the host, so: operators element by element, residuals recomputed by the oracle
+    for sampled shifts, the two largest shifts against independent oracle CGs."""
+    cfg, links, b, shifts, res = li.make_config_inputs(5)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    assert rel_l2(rig.dslash(O, b), rig.lat.dslash(O, b)) <= TOL_OP
+    assert rel_l2(rig.mdagm(E, b), rig.lat.mdagm(cfg.mass, E, b)) <= TOL_OP
+    out = rig.solve(E, b, shifts, res, cfg.tol)
+    assert out["status"] == 0 and out["iterations"] > 1000
+    assert (out["true_res"] <= 1.5 * cfg.tol).all(), out["true_res"]
+    for k in (0, 15):
+        xk = out["x"][k]
+        r = b - (rig.lat.mdagm(cfg.mass, E, xk) + shifts[k] * xk)
+        tr = np.linalg.norm(r) / np.linalg.norm(b)
+        assert tr <= 1.5 * cfg.tol and abs(tr - out["true_res"][k]) <= 1e-2 * tr
+    assert rel_l2(out["y"], np.tensordot(res, out["x"], axes=(0, 0))) <= 1e-14
+    _sampled_shift_check(rig, cfg, b, shifts, out, ks=(15,))
