@@ -1,0 +1,397 @@
+#!/usr/bin/env python
+"""bench.py -- the measurement contract.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 3] [--impl ours|reference]
+
+Metric (BASELINE.json): fp64 staggered Dslash algorithmic HBM GB/s at 32^3 x 8 (config 3), with the
+multishift-CG seconds per solve reported beside it.
+
+One STEP is one pass of the whole hot path over one batch of seeded
+synthetic input already resident in HBM (a1, the gauge ingest, happens once before the timed region
+on the device arm, and inside it on the e2e arm's first step only -- a gauge field serves thousands
+of applies):
+    A. PAIRS x (D_oe, D_eo) back to back, one CUDA graph          (a2, a3)   -> `value`
+    B. PAIRS/2 x M^dag M                                           (a4)
+    C. one multishift-CG solve incl. true residuals and y         (a5, a6)   -> cg.s_per_solve
+`value` = 624*V bytes x (Dslash launches of section A) / (CUDA-event time of section A), summed over
+the K steps.  Inputs (151 MB of links + vectors) are larger than the 126 MB L2, so no explicit L2
+flush is issued between iterations; `roofline.traffic` gives the DRAM bytes ncu measured per launch.
+
+N > 1: the path runs on one GPU with no sharding (BASELINE.json north_star; DESIGN.md "replicas
+only"): every rank runs the same workload independently, no data-path collective; `value` is the
+sum over ranks of algorithmic bytes divided by the slowest rank's time.
+
+`--impl reference` times the CPU oracle as it stands on the host cores (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import lattice_inputs as li  # noqa: E402
+
+METRIC = "staggered_dslash_fp64_algorithmic_GBps"
+UNIT = "GB/s"
+PAIRS = 50                      # (D_oe, D_eo) pairs per step in section A
+FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
+# summarised in profiles/ (None until a capture for that workload exists).
+NCU_DRAM_BYTES_PER_LAUNCH = {3: None, 5: None}
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def dslash_bytes(volume: int) -> int:
+    """Algorithmic bytes of one single-parity Dslash apply: links 576V + in 24V + out 24V
+    (DESIGN.md 'Algorithmic bytes')."""
+    return 624 * volume
+
+
+def dslash_flops(volume: int) -> int:
+    return 285 * volume          # 570 flop per output site
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled every 200 ms during the timed region."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index: int):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, val in zip(self.NAMES, f[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(cfg, links, b, shifts, res, n_pairs: int, cg_iters: int):
+    """Time the oracle as it stands on the host cores on a bounded sample of the workload."""
+    import oracle
+    lat = oracle.Lattice(cfg.dims, links)
+    vo = lat.dslash(1, b)                       # warm-up, also the odd vector
+    t0 = time.perf_counter()
+    for _ in range(n_pairs):
+        vo = lat.dslash(1, b)
+        ve = lat.dslash(0, vo)
+    t_d = time.perf_counter() - t0
+    del ve
+    gbps = 2 * n_pairs * dslash_bytes(cfg.volume) / t_d / 1e9
+    t0 = time.perf_counter()
+    out = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=cg_iters,
+                            want_x=False)
+    t_cg = time.perf_counter() - t0
+    return dict(gbps=gbps, dslash_s=t_d / (2 * n_pairs), cg_s_per_iter=t_cg / max(out["iterations"], 1),
+                cg_iters=out["iterations"], cores=oracle.threads(), seconds=t_d + t_cg)
+
+
+def run_reference(args, cfg, links, b, shifts, res):
+    """--impl reference: the CPU oracle on the host cores; each step is a bounded sample."""
+    import oracle
+    lat = oracle.Lattice(cfg.dims, links)
+    pairs = 2
+    for _ in range(args.warmup):
+        lat.dslash(0, lat.dslash(1, b))
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        for _ in range(pairs):
+            lat.dslash(0, lat.dslash(1, b))
+    t = time.perf_counter() - t0
+    value = args.steps * pairs * 2 * dslash_bytes(cfg.volume) / t / 1e9
+    t0 = time.perf_counter()
+    cg = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=10, want_x=False)
+    t_cg = (time.perf_counter() - t0) / max(cg["iterations"], 1)
+    sample = (f"{pairs} x (D_oe, D_eo) per step on {cfg.name}, all of the lattice; CG: 10 iterations "
+              f"of the {cfg.nshift}-shift solve")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": workload_config(cfg, args),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+                         "sample": sample, "cg_s_per_iteration": t_cg},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, args):
+    nx, ny, nz, nt = cfg.dims
+    return {"workload": f"config {cfg.number}: {nx}^3x{nt} staggered fp64, {cfg.links} SU(3) links"
+                        f"{' eps=%g' % cfg.eps if cfg.eps else ''}, m={cfg.mass}, "
+                        f"{cfg.nshift} shifts in [{cfg.shift_lo:g},{cfg.shift_hi:g}], tol={cfg.tol:g}",
+            "dims": list(cfg.dims), "dslash_pairs_per_step": PAIRS, "mdagm_per_step": PAIRS // 2,
+            "solves_per_step": 1, "l2": "inputs larger than L2 (no explicit flush)",
+            "parallelism": "replicas only" if args.gpus > 1 else "single GPU"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config number (1-5)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-solve", action="store_true", help="skip section C (profiling aid)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        cfg, links, b, shifts, res = li.make_config_inputs(args.workload)
+        run_reference(args, cfg, links, b, shifts, res)
+        return 0
+
+    import torch
+    import paper_1710_09178_b200 as q
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg, links, b, shifts, res = li.make_config_inputs(args.workload)
+    V = cfg.volume
+    stream = torch.cuda.current_stream()
+    ctx = q.Context(cfg.dims, cfg.mass, stream=stream.cuda_stream)
+    d_links = torch.from_numpy(links).cuda()
+    ctx.load_gauge(d_links)
+    torch.cuda.synchronize()
+    del d_links
+
+    d_b, d_o, d_e, d_a = ctx.new_vector(), ctx.new_vector(), ctx.new_vector(), ctx.new_vector()
+    ctx.pack(0, torch.from_numpy(b).cuda().reshape(-1), d_b)
+    d_y = ctx.new_vector()
+
+    # sections A and B as CUDA graphs (launch gaps minimised; the kernels are ~25 us each)
+    def capture(fn):
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            ctx.set_stream(side.cuda_stream)
+            fn()                                   # warm-up outside capture
+            side.synchronize()
+            with torch.cuda.graph(g, stream=side):
+                fn()
+        ctx.set_stream(stream.cuda_stream)
+        torch.cuda.current_stream().wait_stream(side)
+        return g
+
+    def section_a():
+        for _ in range(PAIRS):
+            ctx.dslash(1, d_b, d_o)    # D_oe
+            ctx.dslash(0, d_o, d_e)    # D_eo
+
+    def section_b():
+        for _ in range(PAIRS // 2):
+            ctx.mdagm(0, d_b, d_a)
+
+    graph_a, graph_b = capture(section_a), capture(section_b)
+    launches_a, launches_b = 2 * PAIRS, 2 * (PAIRS // 2)
+
+    def solve():
+        return ctx.multishift_cg(cfg.parity, d_b, shifts, res, cfg.tol, 100000, None, d_y)
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+    t_a = t_b = 0.0
+    t_c = []
+    iters = 0
+    cg_launches = 0
+
+    def step(timed: bool):
+        nonlocal t_a, t_b, iters, cg_launches
+        e0, e1, e2 = ev(), ev(), ev()
+        e0.record()
+        graph_a.replay()
+        e1.record()
+        graph_b.replay()
+        e2.record()
+        if not args.no_solve:
+            l0 = ctx.launch_count
+            w0 = time.perf_counter()
+            st, it, tr = solve()
+            w1 = time.perf_counter()
+            assert st == 0 and tr.max() <= 1.5 * cfg.tol, (st, tr)
+        torch.cuda.synchronize()
+        if timed:
+            t_a += e0.elapsed_time(e1) * 1e-3
+            t_b += e1.elapsed_time(e2) * 1e-3
+            if not args.no_solve:
+                t_c.append(w1 - w0)
+                iters = it
+                cg_launches = ctx.launch_count - l0
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(False)
+    barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    e_start, e_stop = ev(), ev()
+    e_start.record()
+    for _ in range(args.steps):
+        step(True)
+    e_stop.record()
+    barrier()
+    total_s = e_start.elapsed_time(e_stop) * 1e-3
+    clocks = sampler.stop() if sampler else None
+
+    # max over ranks of every timing
+    times = torch.tensor([total_s, t_a, t_b, sum(t_c)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    total_s, t_a, t_b, t_c_sum = times.tolist()
+
+    K = args.steps
+    n = world
+    bytes_a = K * launches_a * dslash_bytes(V)
+    value = n * bytes_a / t_a / 1e9
+    per_launch_s = t_a / (K * launches_a)
+    peak, peak_src = measured_peak()
+    achieved = dslash_bytes(V) / per_launch_s / 1e9
+    mdagm_gbps = n * K * (PAIRS // 2) * 1272 * V / t_b / 1e9
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n, "steps": K, "warmup": args.warmup,
+        "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(cfg, args),
+        "dslash": {"us_per_apply": 1e6 * per_launch_s, "gflops": dslash_flops(V) / per_launch_s / 1e9,
+                   "pct_of_8000": 100 * achieved / 8000.0, "pct_of_measured_peak": 100 * achieved / peak},
+        "mdagm": {"us_per_apply": 1e6 * t_b / (K * (PAIRS // 2)), "GBps_at_1272V": mdagm_gbps},
+        "roofline": {"bound": "hbm", "kernel": "dslash_kernel<false,false> (one D_oe or D_eo apply)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": dslash_bytes(V),
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.number)},
+        "gpu_launches": K * (launches_a + launches_b + cg_launches),
+    }
+    if not args.no_solve:
+        line["cg"] = {"s_per_solve": t_c_sum / K, "iterations": iters,
+                      "us_per_iteration": 1e6 * (t_c_sum / K) / max(iters, 1), "nshift": cfg.nshift,
+                      "tol": cfg.tol, "includes": "true residuals (a6) and y = sum c_k x_k",
+                      "timing": "host wall clock around the blocking C-ABI call"}
+    if clocks is not None:
+        line["clocks"] = clocks
+
+    if rank == 0:
+        # e2e: the same metric through the C ABI with HOST buffers (pinned), copies inside the region
+        hb = torch.from_numpy(b).pin_memory().numpy()
+        ho = torch.empty(b.shape, dtype=torch.float64).pin_memory().numpy()
+        he = torch.empty(b.shape, dtype=torch.float64).pin_memory().numpy()
+        hy = torch.empty(b.shape, dtype=torch.float64).pin_memory().numpy()
+        for _ in range(max(args.warmup, 1)):
+            ctx.dslash_host(1, hb, ho)
+            ctx.dslash_host(0, ho, he)
+        torch.cuda.synchronize()
+        reps = max(K, 5)
+        w0 = time.perf_counter()
+        for _ in range(reps):
+            ctx.dslash_host(1, hb, ho)
+            ctx.dslash_host(0, ho, he)
+        w = time.perf_counter() - w0
+        e2e = {"value": reps * 2 * dslash_bytes(V) / w / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": 2 * b.nbytes, "d2h_bytes_per_step": 2 * b.nbytes,
+               "step": "qcd_dslash_host(D_oe) + qcd_dslash_host(D_eo), pinned host vectors, gauge resident",
+               "us_per_apply": 1e6 * w / (2 * reps)}
+        if not args.no_solve:
+            w0 = time.perf_counter()
+            st, it, tr = ctx.multishift_cg_host(cfg.parity, hb, shifts, res, cfg.tol, 100000, None, hy)
+            e2e["cg_s_per_solve"] = time.perf_counter() - w0
+            e2e["cg_h2d_bytes"] = b.nbytes
+            e2e["cg_d2h_bytes"] = b.nbytes
+        w0 = time.perf_counter()
+        ctx.load_gauge_host(links)
+        e2e["gauge_ingest_s"] = time.perf_counter() - w0
+        e2e["gauge_h2d_bytes"] = links.nbytes
+        line["e2e"] = e2e
+
+        if not args.no_cpu_baseline:
+            pairs = 4 if V <= 262144 else 1
+            smp = oracle_sample(cfg, links, b, shifts, res, n_pairs=pairs, cg_iters=10)
+            line["cpu_baseline"] = {
+                "value": smp["gbps"], "unit": UNIT, "cores": smp["cores"], "kind": "oracle",
+                "sample": f"{pairs} x (D_oe, D_eo) on the full {cfg.name} lattice + 10 iterations of the "
+                          f"{cfg.nshift}-shift CG ({smp['seconds']:.1f} s of host time)",
+                "dslash_us_per_apply": 1e6 * smp["dslash_s"], "cg_s_per_iteration": smp["cg_s_per_iter"],
+                "host_cpu_count": os.cpu_count()}
+        print(json.dumps(line), flush=True)
+
+    ctx.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
