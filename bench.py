@@ -73,6 +73,22 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def max_over_ranks(values, dist=None, device="cpu"):
+    """Element-wise MAX over all ranks of a list of floats (device timings).  `dist` is
+    torch.distributed once initialised (nccl on the GPU box, gloo in the CPU tests) or None."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_rate(world: int, units_per_rank: float, slowest_seconds: float) -> float:
+    """Replicas only: every rank processes `units_per_rank`; the job's rate is
+    all ranks' units over the slowest rank's time."""
+    return world * units_per_rank / slowest_seconds
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons sampled every 200 ms during the timed region."""
 
@@ -191,6 +207,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-solve", action="store_true", help="skip section C (profiling aid)")
+    ap.add_argument("--no-pdl", action="store_true", help="QCD_OPT_PDL=0 (A/B aid)")
+    ap.add_argument("--no-cg-graph", action="store_true", help="QCD_OPT_CG_GRAPH=0 (A/B aid)")
+    ap.add_argument("--cg-batch", type=int, default=0, help="QCD_OPT_CG_BATCH (0 = library default)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -221,6 +240,12 @@ def main():
     V = cfg.volume
     stream = torch.cuda.current_stream()
     ctx = q.Context(cfg.dims, cfg.mass, stream=stream.cuda_stream)
+    if args.no_pdl:
+        ctx.set_option(q.QCD_OPT_PDL, 0)
+    if args.no_cg_graph:
+        ctx.set_option(q.QCD_OPT_CG_GRAPH, 0)
+    if args.cg_batch:
+        ctx.set_option(q.QCD_OPT_CG_BATCH, args.cg_batch)
     d_links = torch.from_numpy(links).cuda()
     ctx.load_gauge(d_links)
     torch.cuda.synchronize()
@@ -276,6 +301,7 @@ def main():
         e2.record()
         if not args.no_solve:
             l0 = ctx.launch_count
+            torch.cuda.synchronize()           # sections A and B are asynchronous: drain them first
             w0 = time.perf_counter()
             st, it, tr = solve()
             w1 = time.perf_counter()
@@ -308,15 +334,12 @@ def main():
     clocks = sampler.stop() if sampler else None
 
     # max over ranks of every timing
-    times = torch.tensor([total_s, t_a, t_b, sum(t_c)], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    total_s, t_a, t_b, t_c_sum = times.tolist()
+    total_s, t_a, t_b, t_c_sum = max_over_ranks([total_s, t_a, t_b, sum(t_c)], dist, "cuda")
 
     K = args.steps
     n = world
     bytes_a = K * launches_a * dslash_bytes(V)
-    value = n * bytes_a / t_a / 1e9
+    value = whole_job_rate(n, bytes_a, t_a) / 1e9
     per_launch_s = t_a / (K * launches_a)
     peak, peak_src = measured_peak()
     achieved = dslash_bytes(V) / per_launch_s / 1e9

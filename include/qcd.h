@@ -70,6 +70,18 @@ QCD_API qcd_status qcd_destroy(qcd_ctx *ctx);
 QCD_API qcd_status qcd_set_mass(qcd_ctx *ctx, double mass);
 QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 
+/* Execution options; none of them changes what is computed.
+ *   QCD_OPT_PDL       (default 1) launch every kernel with programmatic dependent launch, so that its
+ *                     index arithmetic overlaps the tail of its predecessor in the stream or graph.
+ *   QCD_OPT_CG_GRAPH  (default 1) qcd_multishift_cg replays one captured CUDA graph per batch of
+ *                     iterations instead of launching 4 kernels per iteration from the host.
+ *   QCD_OPT_CG_BATCH  (default 8) iterations per batch; the host reads the device's convergence flag
+ *                     once per batch, one batch late, so up to 2 batches of early-exit kernels follow
+ *                     convergence.  1 <= value <= 1024.
+ * Returns QCD_EINVAL for an unknown option or a value out of range. */
+enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2 };
+QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
+
 /* Size in doubles of one internal parity vector: 6 * V/2. */
 QCD_API long qcd_vector_doubles(const qcd_ctx *ctx);
 

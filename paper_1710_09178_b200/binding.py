@@ -15,6 +15,7 @@ import re
 import numpy as np
 
 QCD_EVEN, QCD_ODD = 0, 1
+QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH = 0, 1, 2
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONV, QCD_ESTATE = range(6)
 _STATUS_NAMES = ["QCD_OK", "QCD_EINVAL", "QCD_ENOMEM", "QCD_ECUDA", "QCD_ENOTCONV", "QCD_ESTATE"]
 
@@ -29,6 +30,7 @@ _SIGNATURES = {
     "qcd_destroy": (_ci, [_vp]),
     "qcd_set_mass": (_ci, [_vp, _cd]),
     "qcd_set_stream": (_ci, [_vp, _vp]),
+    "qcd_set_option": (_ci, [_vp, _ci, _cl]),
     "qcd_vector_doubles": (_cl, [_vp]),
     "qcd_load_gauge": (_ci, [_vp, _vp]),
     "qcd_load_gauge_host": (_ci, [_vp, _vp]),
@@ -151,6 +153,9 @@ class Context:
 
     def set_mass(self, mass: float):
         self._check(self._lib.qcd_set_mass(self._h, float(mass)), "qcd_set_mass")
+
+    def set_option(self, option: int, value: int):
+        self._check(self._lib.qcd_set_option(self._h, int(option), int(value)), "qcd_set_option")
 
     def set_stream(self, stream: int):
         self._check(self._lib.qcd_set_stream(self._h, _vp(stream)), "qcd_set_stream")

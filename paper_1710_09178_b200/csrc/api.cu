@@ -39,6 +39,22 @@ struct qcd_ctx {
     double2 *hv_a = nullptr, *hv_b = nullptr, *hv_y = nullptr;   // internal vectors
     long launches = 0;
     std::string err;
+    // options (qcd_set_option)
+    bool opt_pdl = true;                // programmatic dependent launch on every kernel
+    bool opt_cg_graph = true;           // replay one captured graph per batch of CG iterations
+    int opt_cg_batch = 8;               // iterations enqueued per batch / per graph
+    // cached graph of one batch of CG iterations (valid for exactly the key below)
+    cudaGraphExec_t cg_exec = nullptr;
+    cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
+    struct CgKey {
+        int parity = -1, batch = 0; bool pdl = false; double mass = 0.0;
+        const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
+        bool operator==(const CgKey &o) const {
+            return parity == o.parity && batch == o.batch && pdl == o.pdl && mass == o.mass &&
+                   x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
+        }
+    } cg_key;
+    Launch L() const { return Launch{stream, opt_pdl}; }
 };
 
 static std::string g_create_err;
@@ -109,7 +125,48 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->partial;
     p.st = (gated || dot_mode || coeff_from_state) ? c->st : nullptr;
-    c->launches += launch_dslash(c->g, p, c->stream);
+    c->launches += launch_dslash(c->g, p, c->L());
+    return QCD_OK;
+}
+
+// one multishift-CG iteration: 4 kernels, all scalars stay on the device
+void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x)
+{
+    // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
+    run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
+    run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
+    c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->partial, c->st, c->L());
+    c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
+}
+
+// Capture `batch` iterations into a graph (once per distinct set of buffers, parity and mass).
+qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
+{
+    qcd_ctx::CgKey key;
+    key.parity = parity; key.batch = batch; key.pdl = c->opt_pdl; key.mass = c->mass;
+    key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp;
+    if (c->cg_exec && key == c->cg_key) return QCD_OK;
+    if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }
+    if (!c->cap_stream)
+        QCD_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+    cudaStream_t user = c->stream;
+    const long launches0 = c->launches;
+    c->stream = c->cap_stream;
+    cudaError_t e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) {
+        for (int i = 0; i < batch; ++i) enqueue_cg_iteration(c, parity, x);
+        cudaGraph_t graph = nullptr;
+        e = cudaStreamEndCapture(c->cap_stream, &graph);
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+    }
+    c->stream = user;
+    c->launches = launches0;          // capturing launches nothing
+    if (e != cudaSuccess) {
+        c->cg_exec = nullptr;
+        return fail(c, QCD_ECUDA, std::string("CG graph capture: ") + cudaGetErrorString(e));
+    }
+    c->cg_key = key;
     return QCD_OK;
 }
 
@@ -181,6 +238,8 @@ qcd_status qcd_destroy(qcd_ctx *c)
 {
     if (!c) return QCD_OK;
     cudaStreamSynchronize(c->stream);
+    if (c->cg_exec) cudaGraphExecDestroy(c->cg_exec);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaFree(c->W); cudaFree(c->tmp); cudaFree(c->q); cudaFree(c->r); cudaFree(c->p);
     cudaFree(c->xws); cudaFree(c->partial); cudaFree(c->st); cudaFree(c->results);
     cudaFree(c->stage_links); cudaFree(c->stage_vec); cudaFree(c->hv_a); cudaFree(c->hv_b);
@@ -208,6 +267,20 @@ qcd_status qcd_set_stream(qcd_ctx *c, void *cuda_stream)
     return QCD_OK;
 }
 
+qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
+{
+    if (!c) return QCD_EINVAL;
+    switch (option) {
+    case QCD_OPT_PDL: c->opt_pdl = value != 0; return QCD_OK;
+    case QCD_OPT_CG_GRAPH: c->opt_cg_graph = value != 0; return QCD_OK;
+    case QCD_OPT_CG_BATCH:
+        if (value < 1 || value > 1024) return fail(c, QCD_EINVAL, "qcd_set_option: batch must be in [1, 1024]");
+        c->opt_cg_batch = (int)value;
+        return QCD_OK;
+    default: return fail(c, QCD_EINVAL, "qcd_set_option: unknown option");
+    }
+}
+
 long qcd_vector_doubles(const qcd_ctx *c) { return c ? 2 * c->n2 : 0; }
 long qcd_launch_count(const qcd_ctx *c) { return c ? c->launches : 0; }
 const char *qcd_last_error(const qcd_ctx *c) { return c ? c->err.c_str() : g_create_err.c_str(); }
@@ -216,7 +289,7 @@ qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
 {
     if (!c) return QCD_EINVAL;
     if (!d_links) return fail(c, QCD_EINVAL, "qcd_load_gauge: NULL links");
-    c->launches += launch_ingest_links(c->g, d_links, c->W, c->stream);
+    c->launches += launch_ingest_links(c->g, d_links, c->W, c->L());
     qcd_status s = check_launch(c, "qcd_load_gauge");
     if (s == QCD_OK) c->gauge_loaded = true;
     return s;
@@ -240,7 +313,7 @@ qcd_status qcd_pack(qcd_ctx *c, int parity, const double *d_canon, double *d_int
     if (!c) return QCD_EINVAL;
     if (bad_parity(parity) || !d_canon || !d_internal || d_canon == d_internal)
         return fail(c, QCD_EINVAL, "qcd_pack: bad argument");
-    c->launches += launch_pack(c->g, d_canon, (double2 *)d_internal, c->stream);
+    c->launches += launch_pack(c->g, d_canon, (double2 *)d_internal, c->L());
     return check_launch(c, "qcd_pack");
 }
 
@@ -249,7 +322,7 @@ qcd_status qcd_unpack(qcd_ctx *c, int parity, const double *d_internal, double *
     if (!c) return QCD_EINVAL;
     if (bad_parity(parity) || !d_canon || !d_internal || d_canon == d_internal)
         return fail(c, QCD_EINVAL, "qcd_unpack: bad argument");
-    c->launches += launch_unpack(c->g, (const double2 *)d_internal, d_canon, c->stream);
+    c->launches += launch_unpack(c->g, (const double2 *)d_internal, d_canon, c->L());
     return check_launch(c, "qcd_unpack");
 }
 
@@ -320,21 +393,23 @@ qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshi
     h.sigma0 = h.sigma[0];
     QCD_CUDA(c, cudaMemcpyAsync(c->st, &h, sizeof h, cudaMemcpyHostToDevice, st));
     QCD_CUDA(c, cudaMemsetAsync(x, 0, (size_t)n2 * nshift * sizeof(double2), st));
-    c->launches += launch_cg_init(n2, b, c->r, c->p, n2, nshift, c->partial, c->st, st);
+    c->launches += launch_cg_init(n2, b, c->r, c->p, n2, nshift, c->partial, c->st, c->L());
 
-    // iteration loop: enqueue only
-    const int batch = 16;
+    // iteration loop: enqueue only (one graph replay, or 4 launches per iteration, per batch)
+    const int batch = std::max(1, std::min(c->opt_cg_batch, max_iter));
+    const bool use_graph = c->opt_cg_graph;
+    if (use_graph && (s = ensure_cg_graph(c, parity, x, batch)) != QCD_OK) return s;
     int enq = 0, cur = 0;
     bool pending = false, finished = false;
     c->h_done[0] = c->h_done[1] = 0;
     while (!finished && enq < max_iter) {
-        const int nb = std::min(batch, max_iter - enq);
-        for (int i = 0; i < nb; ++i) {
-            // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
-            run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
-            run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
-            c->launches += launch_cg_update_r(n2, c->r, c->q, c->partial, c->st, st);
-            c->launches += launch_cg_update_shifts(n2, c->r, x, c->p, n2, c->st, st);
+        // a graph always holds `batch` iterations; iterations past max_iter exit early on the device
+        const int nb = use_graph ? batch : std::min(batch, max_iter - enq);
+        if (use_graph) {
+            QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));
+            c->launches += 4L * batch;
+        } else {
+            for (int i = 0; i < nb; ++i) enqueue_cg_iteration(c, parity, x);
         }
         enq += nb;
         if (pending) {
@@ -353,10 +428,10 @@ qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshi
         run_dslash(c, 1 - parity, xk, c->tmp, nullptr, 0.0, false, 0, false);
         run_dslash(c, parity, c->tmp, c->q, xk, c->mass * c->mass, false, 0, false);
         c->launches += launch_residual_norm(n2, b, c->q, xk, h.sigma[k], c->partial, c->st,
-                                            c->results + order[k], st);
+                                            c->results + order[k], c->L());
     }
     if (d_y)
-        c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, (double2 *)d_y, st);
+        c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, (double2 *)d_y, c->L());
     s = check_launch(c, "qcd_multishift_cg");
     if (s != QCD_OK) return s;
     QCD_CUDA(c, cudaMemcpyAsync(c->h_results, c->results, nshift * sizeof(double), cudaMemcpyDeviceToHost, st));

@@ -19,6 +19,8 @@ __global__ void __launch_bounds__(kBlock)
 cg_init_kernel(long n2, const double2 *__restrict__ b, double2 *__restrict__ r,
                double2 *__restrict__ p, long pstride, int nshift, double *partial, CgState *st)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     double s = 0.0;
     for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
         const double2 v = __ldg(b + i);
@@ -41,6 +43,8 @@ __global__ void __launch_bounds__(kBlock)
 cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q, double *partial,
                    CgState *st)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     if (st->done) {                       // dead iteration after convergence
         if (blockIdx.x == 0 && threadIdx.x == 0) st->done_prev = 1;
         return;
@@ -64,6 +68,8 @@ __global__ void __launch_bounds__(kBlock)
 cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restrict__ x,
                         double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     if (st->done_prev) return;
     __shared__ double s_a[kMaxShifts], s_z[kMaxShifts], s_b[kMaxShifts];
     __shared__ long long s_x[kMaxShifts], s_p[kMaxShifts];
@@ -102,6 +108,8 @@ residual_norm_kernel(long n2, const double2 *__restrict__ b, const double2 *__re
                      const double2 *__restrict__ x, double sigma, double *partial, CgState *st,
                      double *result)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     double s = 0.0;
     for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
         double2 d = __ldg(b + i);
@@ -127,6 +135,8 @@ struct CombineArgs {
 __global__ void __launch_bounds__(kBlock)
 combine_kernel(long n2, const double2 *__restrict__ x, const CombineArgs a, double2 *__restrict__ y)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
         double2 s = make_double2(0.0, 0.0);
 #pragma unroll 4
@@ -148,41 +158,41 @@ int blas_grid_blocks(long n2)
 }
 
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
-                   double *partial, CgState *st, cudaStream_t s)
+                   double *partial, CgState *st, Launch L)
 {
-    cg_init_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, b, r, p, pstride, nshift, partial, st);
+    launch_kernel(cg_init_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, r, p, pstride, nshift, partial, st);
     return 1;
 }
 
 int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
-                       cudaStream_t s)
+                       Launch L)
 {
-    cg_update_r_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, r, q, partial, st);
+    launch_kernel(cg_update_r_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st);
     return 1;
 }
 
 int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
-                            CgState *st, cudaStream_t s)
+                            CgState *st, Launch L)
 {
-    cg_update_shifts_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, r, x, p, pstride, st);
+    launch_kernel(cg_update_shifts_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, x, p, pstride, st);
     return 1;
 }
 
 int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
-                         double *partial, CgState *st, double *result, cudaStream_t s)
+                         double *partial, CgState *st, double *result, Launch L)
 {
-    residual_norm_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, b, q, x, sigma, partial, st,
+    launch_kernel(residual_norm_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, q, x, sigma, partial, st,
                                                                  result);
     return 1;
 }
 
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
-                   int nshift, double2 *y, cudaStream_t s)
+                   int nshift, double2 *y, Launch L)
 {
     CombineArgs a;
     a.n = nshift;
     for (int k = 0; k < nshift; ++k) { a.xoff[k] = xoff_host[k]; a.c[k] = residues[k]; }
-    combine_kernel<<<blas_grid_blocks(n2), kBlock, 0, s>>>(n2, x, a, y);
+    launch_kernel(combine_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, x, a, y);
     return 1;
 }
 

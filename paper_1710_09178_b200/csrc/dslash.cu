@@ -38,20 +38,18 @@ template <bool XPAY, bool DOT>
 __global__ void __launch_bounds__(kBlock)
 dslash_kernel(const Geom g, const DslashParams p)
 {
-    if (p.st != nullptr && p.st->done) return;   // CG already converged: dead iteration
     const int Vh = g.Vh;
     const uint32_t h = blockIdx.x * kBlock + threadIdx.x;
     const bool valid = h < (uint32_t)Vh;
     double dot = 0.0;
+    const int par = p.out_parity;
+    int hp[4], hm[4];   // half indices of the 8 neighbours (all of the opposite parity)
     if (valid) {
         uint32_t q, xh, y, z, t;
         g.dxh.divmod(h, q, xh);
         g.dy.divmod(q, q, y);
         g.dz.divmod(q, t, z);
-        const int par = p.out_parity;
         const int r = (y + z + t + par) & 1;      // x = 2*xh + r
-        // half indices of the 8 neighbours (all of the opposite parity)
-        int hp[4], hm[4];
         {
             const int xh_p = r ? ((int)xh + 1 == g.Nxh ? 0 : (int)xh + 1) : (int)xh;
             const int xh_m = r ? (int)xh : (xh == 0 ? g.Nxh - 1 : (int)xh - 1);
@@ -64,6 +62,12 @@ dslash_kernel(const Geom g, const DslashParams p)
             hp[3] = (int)h + ((int)t + 1 == g.Nt ? -(g.Nt - 1) * g.st : g.st);
             hm[3] = (int)h + (t == 0 ? (g.Nt - 1) * g.st : -g.st);
         }
+    }
+    // everything above is index arithmetic; from here on data of the preceding kernel is read
+    pdl_wait();
+    pdl_launch_dependents();
+    if (p.st != nullptr && p.st->done) return;   // CG already converged: dead iteration
+    if (valid) {
         const double2 *__restrict__ in = p.in;
         double2 acc[3];
         acc[0] = acc[1] = acc[2] = make_double2(0.0, 0.0);
@@ -115,15 +119,15 @@ dslash_kernel(const Geom g, const DslashParams p)
 
 int dslash_grid_blocks(const Geom &g) { return (g.Vh + kBlock - 1) / kBlock; }
 
-int launch_dslash(const Geom &g, const DslashParams &p, cudaStream_t s)
+int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
 {
     const int blocks = dslash_grid_blocks(g);
     if (p.src == nullptr)
-        dslash_kernel<false, false><<<blocks, kBlock, 0, s>>>(g, p);
+        launch_kernel(dslash_kernel<false, false>, blocks, kBlock, L.s, L.pdl, g, p);
     else if (p.dot_mode == 0)
-        dslash_kernel<true, false><<<blocks, kBlock, 0, s>>>(g, p);
+        launch_kernel(dslash_kernel<true, false>, blocks, kBlock, L.s, L.pdl, g, p);
     else
-        dslash_kernel<true, true><<<blocks, kBlock, 0, s>>>(g, p);
+        launch_kernel(dslash_kernel<true, true>, blocks, kBlock, L.s, L.pdl, g, p);
     return 1;
 }
 

@@ -58,11 +58,47 @@ struct CgState {
     double scratch;               // generic reduction result (norms for true residuals)
 };
 
-// ---- launchers (each enqueues on `s` and returns the number of kernels launched) ----
+// ---- programmatic dependent launch (PDL) ----
+// Every kernel of the library is launched with cudaLaunchAttributeProgrammaticStreamSerialization
+// (unless switched off by QCD_OPT_PDL): it may become resident while its predecessor in the stream
+// (or graph) is still draining, runs its index arithmetic, and blocks in pdl_wait() until the
+// predecessor has completed and its writes are visible.  Rules kept by every kernel: nothing written
+// and nothing produced by an earlier kernel read before pdl_wait(); pdl_launch_dependents() only
+// after pdl_wait(), so completion is transitive along the chain.
+#ifdef __CUDACC__
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents()
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
 
-int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, cudaStream_t s);
-int launch_pack(const Geom &g, const double *canon, double2 *internal, cudaStream_t s);
-int launch_unpack(const Geom &g, const double2 *internal, double *canon, cudaStream_t s);
+template <class... KArgs, class... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s,
+                                 bool pdl, Args... args)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1u : 0u;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
+
+// ---- launchers (each enqueues on `s` and returns the number of kernels launched) ----
+struct Launch {
+    cudaStream_t s;
+    bool pdl;
+};
+
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, Launch L);
+int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L);
+int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L);
 
 struct DslashParams {
     const double2 *W;
@@ -79,21 +115,21 @@ struct DslashParams {
     double *partial;
     CgState *st;               // also the early-exit flag when non-null
 };
-int launch_dslash(const Geom &g, const DslashParams &p, cudaStream_t s);
+int launch_dslash(const Geom &g, const DslashParams &p, Launch L);
 int dslash_grid_blocks(const Geom &g);
 
 // BLAS-1 (n2 = 3*Vh double2 elements per vector)
 int blas_grid_blocks(long n2);
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
-                   double *partial, CgState *st, cudaStream_t s);
+                   double *partial, CgState *st, Launch L);
 int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
-                       cudaStream_t s);
+                       Launch L);
 int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
-                            CgState *st, cudaStream_t s);
+                            CgState *st, Launch L);
 // scratch = || b - (q + sigma x) ||^2   and  scratch = ||b||^2
 int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
-                         double *partial, CgState *st, double *result, cudaStream_t s);
+                         double *partial, CgState *st, double *result, Launch L);
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
-                   int nshift, double2 *y, cudaStream_t s);
+                   int nshift, double2 *y, Launch L);
 
 }  // namespace qcd

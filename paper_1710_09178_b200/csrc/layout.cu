@@ -16,6 +16,8 @@ constexpr int kBlock = 256;
 __global__ void __launch_bounds__(kBlock)
 ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__ W)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     const int Vh = g.Vh;
     uint32_t tid = blockIdx.x * kBlock + threadIdx.x;
     if (tid >= 2u * Vh) return;
@@ -48,6 +50,8 @@ ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__
 __global__ void __launch_bounds__(kBlock)
 pack_kernel(int Vh, const double2 *__restrict__ canon, double2 *__restrict__ v)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     int h = blockIdx.x * kBlock + threadIdx.x;
     if (h >= Vh) return;
 #pragma unroll
@@ -57,6 +61,8 @@ pack_kernel(int Vh, const double2 *__restrict__ canon, double2 *__restrict__ v)
 __global__ void __launch_bounds__(kBlock)
 unpack_kernel(int Vh, const double2 *__restrict__ v, double2 *__restrict__ canon)
 {
+    pdl_wait();
+    pdl_launch_dependents();
     int h = blockIdx.x * kBlock + threadIdx.x;
     if (h >= Vh) return;
 #pragma unroll
@@ -65,24 +71,24 @@ unpack_kernel(int Vh, const double2 *__restrict__ v, double2 *__restrict__ canon
 
 }  // namespace
 
-int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, cudaStream_t s)
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, Launch L)
 {
     int blocks = (2 * g.Vh + kBlock - 1) / kBlock;
-    ingest_links_kernel<<<blocks, kBlock, 0, s>>>(g, (const double2 *)links_canon, W);
+    launch_kernel(ingest_links_kernel, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W);
     return 1;
 }
 
-int launch_pack(const Geom &g, const double *canon, double2 *internal, cudaStream_t s)
+int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L)
 {
     int blocks = (g.Vh + kBlock - 1) / kBlock;
-    pack_kernel<<<blocks, kBlock, 0, s>>>(g.Vh, (const double2 *)canon, internal);
+    launch_kernel(pack_kernel, blocks, kBlock, L.s, L.pdl, g.Vh, (const double2 *)canon, internal);
     return 1;
 }
 
-int launch_unpack(const Geom &g, const double2 *internal, double *canon, cudaStream_t s)
+int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L)
 {
     int blocks = (g.Vh + kBlock - 1) / kBlock;
-    unpack_kernel<<<blocks, kBlock, 0, s>>>(g.Vh, internal, (double2 *)canon);
+    launch_kernel(unpack_kernel, blocks, kBlock, L.s, L.pdl, g.Vh, internal, (double2 *)canon);
     return 1;
 }
 

@@ -178,6 +178,27 @@ def test_multishift_cg_is_deterministic(torch, q):
     assert np.array_equal(o1["x"], o2["x"]) and np.array_equal(o1["y"], o2["y"])
 
 
+def test_execution_options_do_not_change_a_single_bit(torch, q):
+    """QCD_OPT_PDL / QCD_OPT_CG_GRAPH / QCD_OPT_CG_BATCH only change how work is enqueued."""
+    cfg, links, b, shifts, res = li.make_config_inputs(2)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    ref = rig.solve(E, b, shifts, res, cfg.tol)
+    ref_d = rig.dslash(O, b)
+    for pdl, graph, batch in [(0, 0, 16), (1, 0, 3), (0, 1, 1), (1, 1, 5), (1, 1, 64)]:
+        rig.ctx.set_option(q.QCD_OPT_PDL, pdl)
+        rig.ctx.set_option(q.QCD_OPT_CG_GRAPH, graph)
+        rig.ctx.set_option(q.QCD_OPT_CG_BATCH, batch)
+        out = rig.solve(E, b, shifts, res, cfg.tol)
+        assert out["iterations"] == ref["iterations"] and out["status"] == 0
+        assert np.array_equal(out["x"], ref["x"]) and np.array_equal(out["y"], ref["y"])
+        assert np.array_equal(out["true_res"], ref["true_res"])
+        assert np.array_equal(rig.dslash(O, b), ref_d)
+    with pytest.raises(q.QcdError):
+        rig.ctx.set_option(q.QCD_OPT_CG_BATCH, 0)
+    with pytest.raises(q.QcdError):
+        rig.ctx.set_option(99, 1)
+
+
 def test_multishift_cg_odd_parity_unsorted_shifts_zero_shift(torch, q):
     dims, mass = (4, 6, 4, 4), 0.08
     rig = make_rig(torch, q, dims, "random", mass, 7)
