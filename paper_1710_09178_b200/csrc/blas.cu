@@ -12,7 +12,7 @@ namespace qcd {
 namespace {
 
 constexpr int kBlock = 256;
-constexpr int kMaxBlocks = 148 * 8;   // grid-stride above this: a multiple of the SM count
+constexpr int kMaxBlocks = 148 * 16;  // grid-stride above this: a multiple of the SM count
 
 // r = b ; p_k = b (all k) ; rho = rho_b = <b,b> ; x_k are zeroed by a memset
 __global__ void __launch_bounds__(kBlock)
@@ -64,6 +64,14 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
 }
 
 // for every shift k updated this iteration:  x_k += alpha_k p_k ;  p_k = zeta_k^new r + beta_k p_k
+// ("the heaviest kernel which updates three large arrays").  Work is cut into units of
+// (chunk of kShiftChunk elements, shift): unit u -> shift u % nl, chunk u / nl, dealt round-robin to
+// the CTAs, so the load per SM is even for any number of active shifts and any lattice size, and the
+// CTAs that share a chunk of r run next to each other (L2).  Each thread streams kShiftUnroll
+// independent (x, p) pairs per unit.
+constexpr int kShiftUnroll = 4;
+constexpr int kShiftChunk = kBlock * kShiftUnroll;
+
 __global__ void __launch_bounds__(kBlock)
 cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restrict__ x,
                         double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
@@ -83,21 +91,31 @@ cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restr
         s_p[threadIdx.x] = (long long)k * pstride;
     }
     __syncthreads();
-    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
-        const double2 rv = __ldg(r + i);
-#pragma unroll 4
-        for (int j = 0; j < nl; ++j) {
-            double2 *xp = x + s_x[j] + i;
-            double2 *pp = p + s_p[j] + i;
-            double2 xv = *xp;
-            double2 pv = *pp;
-            const double a = s_a[j], z = s_z[j], bb = s_b[j];
-            xv.x = fma(a, pv.x, xv.x);
-            xv.y = fma(a, pv.y, xv.y);
-            pv.x = fma(bb, pv.x, z * rv.x);
-            pv.y = fma(bb, pv.y, z * rv.y);
-            *xp = xv;
-            *pp = pv;
+    const unsigned nchunk = (unsigned)((n2 + kShiftChunk - 1) / kShiftChunk);
+    const unsigned nunit = nchunk * (unsigned)nl;
+    for (unsigned u = blockIdx.x; u < nunit; u += gridDim.x) {
+        const unsigned c = u / (unsigned)nl, j = u - c * (unsigned)nl;
+        const long base = (long)c * kShiftChunk + threadIdx.x;
+        double2 *__restrict__ xp = x + s_x[j];
+        double2 *__restrict__ pp = p + s_p[j];
+        const double a = s_a[j], z = s_z[j], bb = s_b[j];
+        double2 rv[kShiftUnroll], xv[kShiftUnroll], pv[kShiftUnroll];
+#pragma unroll
+        for (int e = 0; e < kShiftUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) { xv[e] = xp[i]; pv[e] = pp[i]; rv[e] = __ldg(r + i); }
+        }
+#pragma unroll
+        for (int e = 0; e < kShiftUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) {
+                xv[e].x = fma(a, pv[e].x, xv[e].x);
+                xv[e].y = fma(a, pv[e].y, xv[e].y);
+                pv[e].x = fma(bb, pv[e].x, z * rv[e].x);
+                pv[e].y = fma(bb, pv[e].y, z * rv[e].y);
+                xp[i] = xv[e];
+                pp[i] = pv[e];
+            }
         }
     }
 }
@@ -174,7 +192,10 @@ int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, C
 int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
                             CgState *st, Launch L)
 {
-    launch_kernel(cg_update_shifts_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, x, p, pstride, st);
+    // the number of active shifts is only known on the device: size the grid for all of them
+    long units = (n2 + kShiftChunk - 1) / kShiftChunk * kMaxShifts;
+    int grid = (int)(units < 148 * 8 ? (units > 0 ? units : 1) : 148 * 8);
+    launch_kernel(cg_update_shifts_kernel, grid, kBlock, L.s, L.pdl, n2, r, x, p, pstride, st);
     return 1;
 }
 
