@@ -183,3 +183,39 @@ class Lattice:
             tr[k] = self.polish(mass, parity, shifts[k], b, x[k], max_iter=max_iter)
         y = np.tensordot(residues, x, axes=(0, 0))
         return dict(x=x, y=y, true_res=tr, iterations=out["iterations"])
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1: two-row link storage.  PAPER.md:168: "one often stores and moves only
+# two rows (or columns) of the (3 x 3) complex link matrix and recovers the third by
+# orthogonalization.  This is often known as data compression."  For U in SU(3) the rows are
+# orthonormal and det U = 1, which fixes the third row uniquely: row_2 = conj(row_0 x row_1)
+# (the complex cross product).  The definition is written out below with plain numpy; the
+# operator itself is unchanged, so the oracle for the compressed Dslash is Lattice(...) built on
+# reconstruct_links_2row(compress_links_2row(U)).
+# Pins (tests/test_oracle_compression.py): hand-written SU(3) matrices (diagonal phases, a cyclic
+# permutation, a real rotation), det/unitarity of the result for arbitrary orthonormal rows,
+# identity with the input on the seeded SU(3) generators.
+
+def compress_links_2row(links: np.ndarray) -> np.ndarray:
+    """float64[V,4,3,3,2] -> float64[V,4,2,3,2]: rows 0 and 1 of every link, bit for bit."""
+    links = _f64(links)
+    v = links.size // 72
+    return np.ascontiguousarray(links.reshape(v, 4, 3, 3, 2)[:, :, :2])
+
+
+def reconstruct_links_2row(rows: np.ndarray) -> np.ndarray:
+    """float64[V,4,2,3,2] -> float64[V,4,3,3,2] with row_2 = conj(row_0 x row_1), i.e.
+    row_2[c] = conj(row_0[c+1] row_1[c+2] - row_0[c+2] row_1[c+1]), indices mod 3."""
+    rows = _f64(rows)
+    a = rows[:, :, 0, :, 0] + 1j * rows[:, :, 0, :, 1]      # row 0: complex[V,4,3]
+    b = rows[:, :, 1, :, 0] + 1j * rows[:, :, 1, :, 1]      # row 1
+    third = np.empty_like(a)
+    for c in range(3):
+        c1, c2 = (c + 1) % 3, (c + 2) % 3
+        third[:, :, c] = np.conj(a[:, :, c1] * b[:, :, c2] - a[:, :, c2] * b[:, :, c1])
+    out = np.empty(rows.shape[:2] + (3, 3, 2))
+    out[:, :, :2] = rows
+    out[:, :, 2, :, 0] = third.real
+    out[:, :, 2, :, 1] = third.imag
+    return out
