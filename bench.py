@@ -47,7 +47,7 @@ PAIRS = 50                      # (D_oe, D_eo) pairs per step in section A
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
 # summarised in profiles/ (None until a capture for that workload exists).
-NCU_DRAM_BYTES_PER_LAUNCH = {3: None, 5: None}
+NCU_DRAM_BYTES_PER_LAUNCH = {3: 163.3e6, 5: None}   # profiles/r01_dslash_full_cfg3.md
 
 
 def log(*a):
