@@ -47,17 +47,18 @@ PAIRS = 50                      # (D_oe, D_eo) pairs per step in section A
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
 # summarised in profiles/ (None until a capture for that workload exists).
-NCU_DRAM_BYTES_PER_LAUNCH = {3: 163.3e6, 5: None}   # profiles/r01_dslash_full_cfg3.md
+# key: (config number, link rows)
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 163.3e6}   # profiles/r01_dslash_full_cfg3.md
 
 
 def log(*a):
     print(*a, file=sys.stderr, flush=True)
 
 
-def dslash_bytes(volume: int) -> int:
+def dslash_bytes(volume: int, link_rows: int = 3) -> int:
     """Algorithmic bytes of one single-parity Dslash apply: links 576V + in 24V + out 24V
-    (DESIGN.md 'Algorithmic bytes')."""
-    return 624 * volume
+    (DESIGN.md 'Algorithmic bytes'); two-row storage moves 384V of links."""
+    return (624 if link_rows == 3 else 432) * volume
 
 
 def dslash_flops(volume: int) -> int:
@@ -210,6 +211,10 @@ def main():
     ap.add_argument("--no-pdl", action="store_true", help="QCD_OPT_PDL=0 (A/B aid)")
     ap.add_argument("--no-cg-graph", action="store_true", help="QCD_OPT_CG_GRAPH=0 (A/B aid)")
     ap.add_argument("--cg-batch", type=int, default=0, help="QCD_OPT_CG_BATCH (0 = library default)")
+    ap.add_argument("--link-rows", type=int, default=3, choices=[2, 3],
+                    help="QCD_OPT_LINK_ROWS for the whole run (default 3, the paper's uncompressed "
+                         "storage; the default run also reports a two-row section)")
+    ap.add_argument("--no-two-row", action="store_true", help="skip the extra two-row section")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -246,6 +251,7 @@ def main():
         ctx.set_option(q.QCD_OPT_CG_GRAPH, 0)
     if args.cg_batch:
         ctx.set_option(q.QCD_OPT_CG_BATCH, args.cg_batch)
+    ctx.set_option(q.QCD_OPT_LINK_ROWS, args.link_rows)
     d_links = torch.from_numpy(links).cuda()
     ctx.load_gauge(d_links)
     torch.cuda.synchronize()
@@ -338,12 +344,14 @@ def main():
 
     K = args.steps
     n = world
-    bytes_a = K * launches_a * dslash_bytes(V)
+    R = args.link_rows
+    bytes_a = K * launches_a * dslash_bytes(V, R)
     value = whole_job_rate(n, bytes_a, t_a) / 1e9
     per_launch_s = t_a / (K * launches_a)
     peak, peak_src = measured_peak()
-    achieved = dslash_bytes(V) / per_launch_s / 1e9
-    mdagm_gbps = n * K * (PAIRS // 2) * 1272 * V / t_b / 1e9
+    achieved = dslash_bytes(V, R) / per_launch_s / 1e9
+    mdagm_bytes = 2 * dslash_bytes(V, R) + 24 * V
+    mdagm_gbps = n * K * (PAIRS // 2) * mdagm_bytes / t_b / 1e9
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n, "steps": K, "warmup": args.warmup,
@@ -352,11 +360,11 @@ def main():
         "config": workload_config(cfg, args),
         "dslash": {"us_per_apply": 1e6 * per_launch_s, "gflops": dslash_flops(V) / per_launch_s / 1e9,
                    "pct_of_8000": 100 * achieved / 8000.0, "pct_of_measured_peak": 100 * achieved / peak},
-        "mdagm": {"us_per_apply": 1e6 * t_b / (K * (PAIRS // 2)), "GBps_at_1272V": mdagm_gbps},
+        "mdagm": {"us_per_apply": 1e6 * t_b / (K * (PAIRS // 2)), "GBps": mdagm_gbps, "algorithmic_bytes": mdagm_bytes},
         "roofline": {"bound": "hbm", "kernel": "dslash_kernel<false,false> (one D_oe or D_eo apply)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": dslash_bytes(V),
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(cfg.number)},
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": dslash_bytes(V, R), "link_rows": R,
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((cfg.number, R))},
         "gpu_launches": K * (launches_a + launches_b + cg_launches),
     }
     if not args.no_solve:
@@ -383,7 +391,7 @@ def main():
             ctx.dslash_host(1, hb, ho)
             ctx.dslash_host(0, ho, he)
         w = time.perf_counter() - w0
-        e2e = {"value": reps * 2 * dslash_bytes(V) / w / 1e9, "unit": UNIT,
+        e2e = {"value": reps * 2 * dslash_bytes(V, R) / w / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": 2 * b.nbytes, "d2h_bytes_per_step": 2 * b.nbytes,
                "step": "qcd_dslash_host(D_oe) + qcd_dslash_host(D_eo), pinned host vectors, gauge resident",
                "us_per_apply": 1e6 * w / (2 * reps)}
@@ -398,6 +406,39 @@ def main():
         e2e["gauge_ingest_s"] = time.perf_counter() - w0
         e2e["gauge_h2d_bytes"] = links.nbytes
         line["e2e"] = e2e
+
+        if R == 3 and not args.no_two_row:
+            # the same sections A and C with two-row link storage
+            ctx.set_option(q.QCD_OPT_LINK_ROWS, 2)
+            ctx.load_gauge_host(links)
+            graph_a2 = capture(section_a)
+            for _ in range(max(args.warmup, 1)):
+                graph_a2.replay()
+            torch.cuda.synchronize()
+            e0, e1 = ev(), ev()
+            e0.record()
+            for _ in range(K):
+                graph_a2.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            t2 = e0.elapsed_time(e1) * 1e-3 / (K * launches_a)
+            two = {"link_rows": 2, "us_per_apply": 1e6 * t2,
+                   "GBps_at_432V": dslash_bytes(V, 2) / t2 / 1e9,
+                   "frac_of_peak": dslash_bytes(V, 2) / t2 / 1e9 / peak,
+                   "gflops": (285 + 168) * V / t2 / 1e9,
+                   "speedup_vs_three_row": per_launch_s / t2}
+            if not args.no_solve:
+                ts = []
+                for _ in range(max(1, min(K, 3)) + 1):
+                    torch.cuda.synchronize()
+                    w0 = time.perf_counter()
+                    st, it, tr = solve()
+                    ts.append(time.perf_counter() - w0)
+                    assert st == 0 and tr.max() <= 1.5 * cfg.tol, (st, tr)
+                two["cg_s_per_solve"] = statistics.median(ts[1:])
+                two["cg_iterations"] = it
+            line["two_row"] = two
+            ctx.set_option(q.QCD_OPT_LINK_ROWS, 3)
 
         if not args.no_cpu_baseline:
             pairs = 4 if V <= 262144 else 1

@@ -70,7 +70,7 @@ QCD_API qcd_status qcd_destroy(qcd_ctx *ctx);
 QCD_API qcd_status qcd_set_mass(qcd_ctx *ctx, double mass);
 QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 
-/* Execution options; none of them changes what is computed.
+/* Execution options.  The first three do not change a single bit of any result.
  *   QCD_OPT_PDL       (default 1) launch every kernel with programmatic dependent launch, so that its
  *                     index arithmetic overlaps the tail of its predecessor in the stream or graph.
  *   QCD_OPT_CG_GRAPH  (default 1) qcd_multishift_cg replays one captured CUDA graph per batch of
@@ -78,8 +78,15 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *   QCD_OPT_CG_BATCH  (default 8) iterations per batch; the host reads the device's convergence flag
  *                     once per batch, one batch late, so up to 2 batches of early-exit kernels follow
  *                     convergence.  1 <= value <= 1024.
+ *   QCD_OPT_LINK_ROWS (default 3) how the NEXT qcd_load_gauge stores the links.  3: all nine entries
+ *                     (576 V bytes, "72V double precision words").  2: two-row storage
+ *                     (384 V bytes): "one often stores and moves only two rows ... of the (3 x 3)
+ *                     complex link matrix and recovers the third by orthogonalization";
+ *                     the stencil rebuilds row_2 = conj(row_0 x row_1) in registers.  REQUIRES links in
+ *                     SU(3) (unitary, det = 1): rows 2 of the input are ignored.  Results differ from
+ *                     the 3-row path at rounding level only (relative 1e-15) for SU(3) input.
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
-enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2 };
+enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

@@ -38,7 +38,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".{os.getpid()}.tmp"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + sources()
+    extra = os.environ.get("QCD_NVCC_EXTRA", "").split()       # e.g. -DQCD_DSLASH2_MINB=6 (tuning aid)
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + sources()
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
     return LIB

@@ -20,8 +20,10 @@ struct qcd_ctx {
     int device = 0;
     long n2 = 0;              // double2 elements per internal vector = 3*Vh
     size_t vec_bytes = 0;     // bytes of one parity vector (either layout)
-    double2 *W = nullptr;     // [2][4][9][Vh]
+    double2 *W = nullptr;     // [2][4][9][Vh] (3-row) or [2][4][6][Vh] (2-row) in the same buffer
     bool gauge_loaded = false;
+    int link_rows = 3;        // layout of the LOADED field
+    int opt_link_rows = 3;    // layout the next qcd_load_gauge will build
     // workspace (grow-only, freed by qcd_destroy)
     double2 *tmp = nullptr, *q = nullptr, *r = nullptr;
     double2 *p = nullptr;  int p_cap = 0;
@@ -47,10 +49,10 @@ struct qcd_ctx {
     cudaGraphExec_t cg_exec = nullptr;
     cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
     struct CgKey {
-        int parity = -1, batch = 0; bool pdl = false; double mass = 0.0;
+        int parity = -1, batch = 0, rows = 0; bool pdl = false; double mass = 0.0;
         const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
         bool operator==(const CgKey &o) const {
-            return parity == o.parity && batch == o.batch && pdl == o.pdl && mass == o.mass &&
+            return parity == o.parity && batch == o.batch && rows == o.rows && pdl == o.pdl && mass == o.mass &&
                    x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
         }
     } cg_key;
@@ -120,7 +122,7 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
                       bool gated)
 {
     DslashParams p{};
-    p.W = c->W; p.in = in; p.out = out; p.out_parity = out_parity;
+    p.W = c->W; p.link_rows = c->link_rows; p.in = in; p.out = out; p.out_parity = out_parity;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->partial;
@@ -143,7 +145,7 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x)
 qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
 {
     qcd_ctx::CgKey key;
-    key.parity = parity; key.batch = batch; key.pdl = c->opt_pdl; key.mass = c->mass;
+    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.pdl = c->opt_pdl; key.mass = c->mass;
     key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp;
     if (c->cg_exec && key == c->cg_key) return QCD_OK;
     if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }
@@ -277,6 +279,10 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         if (value < 1 || value > 1024) return fail(c, QCD_EINVAL, "qcd_set_option: batch must be in [1, 1024]");
         c->opt_cg_batch = (int)value;
         return QCD_OK;
+    case QCD_OPT_LINK_ROWS:
+        if (value != 2 && value != 3) return fail(c, QCD_EINVAL, "qcd_set_option: link rows must be 2 or 3");
+        c->opt_link_rows = (int)value;
+        return QCD_OK;
     default: return fail(c, QCD_EINVAL, "qcd_set_option: unknown option");
     }
 }
@@ -289,9 +295,9 @@ qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
 {
     if (!c) return QCD_EINVAL;
     if (!d_links) return fail(c, QCD_EINVAL, "qcd_load_gauge: NULL links");
-    c->launches += launch_ingest_links(c->g, d_links, c->W, c->L());
+    c->launches += launch_ingest_links(c->g, d_links, c->W, c->opt_link_rows, c->L());
     qcd_status s = check_launch(c, "qcd_load_gauge");
-    if (s == QCD_OK) c->gauge_loaded = true;
+    if (s == QCD_OK) { c->gauge_loaded = true; c->link_rows = c->opt_link_rows; }
     return s;
 }
 

@@ -16,6 +16,10 @@ namespace qcd {
 namespace {
 
 constexpr int kBlock = 128;
+// minimum resident CTAs per SM asked of ptxas for the two-row kernel (caps its registers)
+#ifndef QCD_DSLASH2_MINB
+#define QCD_DSLASH2_MINB 7   // measured on B200: 7 beats 1, 6, 8 at 32^3x8 (whole grid resident in one wave)
+#endif
 
 // acc += w * v
 __device__ __forceinline__ void cmad(double2 &acc, const double2 w, const double2 v)
@@ -34,16 +38,48 @@ __device__ __forceinline__ void cmsub_conj(double2 &acc, const double2 w, const 
     acc.y = fma(w.y, v.x, acc.y);
 }
 
-template <bool XPAY, bool DOT>
-__global__ void __launch_bounds__(kBlock)
+// x -> -x when neg (sign-bit flip on the integer pipe; the fp64 pipe stays free for the stencil)
+__device__ __forceinline__ double flip(double x, int neg)
+{
+    return __hiloint2double(__double2hiint(x) ^ (neg << 31), __double2loint(x));
+}
+
+// Two-row storage ("stores and moves only two rows ... recovers the
+// third by orthogonalization"): for U in SU(3), row_2 = conj(row_0 x row_1).  u[0..5] hold rows 0, 1.
+__device__ __forceinline__ void third_row(double2 *u)
+{
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+        const double2 a1 = u[c1], a2 = u[c2], b1 = u[3 + c1], b2 = u[3 + c2];
+        double tx = a1.x * b2.x;
+        tx = fma(-a1.y, b2.y, tx);
+        tx = fma(-a2.x, b1.x, tx);
+        tx = fma(a2.y, b1.y, tx);
+        double ty = a1.x * b2.y;
+        ty = fma(a1.y, b2.x, ty);
+        ty = fma(-a2.x, b1.y, ty);
+        ty = fma(-a2.y, b1.x, ty);
+        u[6 + c] = make_double2(tx, -ty);
+    }
+}
+
+// ROWS == 3: W holds 1/2 eta s+ U (all nine entries, signs folded in at ingest).
+// ROWS == 2: W holds rows 0 and 1 of the plain U; eta_mu(x), the t-seam sign and the 1/2 are applied
+//            here.  All of them depend on the OUTPUT site only: eta_mu does not depend on x_mu, and
+//            the seam sign of the backward hop is s-_mu(x).
+template <bool XPAY, bool DOT, int ROWS>
+__global__ void __launch_bounds__(kBlock, ROWS == 2 ? QCD_DSLASH2_MINB : 1)
 dslash_kernel(const Geom g, const DslashParams p)
 {
+    constexpr int NW = 3 * ROWS;
     const int Vh = g.Vh;
     const uint32_t h = blockIdx.x * kBlock + threadIdx.x;
     const bool valid = h < (uint32_t)Vh;
     double dot = 0.0;
     const int par = p.out_parity;
     int hp[4], hm[4];   // half indices of the 8 neighbours (all of the opposite parity)
+    int nf[4] = {0, 0, 0, 0}, nb[4] = {0, 0, 0, 0};   // ROWS == 2: 1 where the hop carries a minus sign
     if (valid) {
         uint32_t q, xh, y, z, t;
         g.dxh.divmod(h, q, xh);
@@ -62,6 +98,14 @@ dslash_kernel(const Geom g, const DslashParams p)
             hp[3] = (int)h + ((int)t + 1 == g.Nt ? -(g.Nt - 1) * g.st : g.st);
             hm[3] = (int)h + (t == 0 ? (g.Nt - 1) * g.st : -g.st);
         }
+        if (ROWS == 2) {
+            const int x = 2 * (int)xh + r;
+            nf[1] = nb[1] = x & 1;                       // eta_1 = (-1)^x
+            nf[2] = nb[2] = (x + (int)y) & 1;            // eta_2 = (-1)^(x+y)
+            const int e3 = (x + (int)y + (int)z) & 1;    // eta_3 = (-1)^(x+y+z)
+            nf[3] = e3 ^ ((int)t + 1 == g.Nt);           // s+ on the hop t = Nt-1 -> 0  (C5)
+            nb[3] = e3 ^ (t == 0);                       // s- on the hop t = 0 -> Nt-1
+        }
     }
     // everything above is index arithmetic; from here on data of the preceding kernel is read
     pdl_wait();
@@ -74,26 +118,43 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             {   // forward hop: + W_mu(x) in(x+mu), link based at x (parity par)
-                const double2 *__restrict__ w = p.W + ((long)(par * 4 + mu) * 9) * Vh + h;
-                double2 v[3];
+                const double2 *__restrict__ w = p.W + ((long)(par * 4 + mu) * NW) * Vh + h;
+                double2 u[9], v[3];
+#pragma unroll
+                for (int i = 0; i < NW; ++i) u[i] = __ldg(w + (long)i * Vh);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hp[mu]);
+                if (ROWS == 2) {
+                    third_row(u);
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) v[c] = make_double2(flip(v[c].x, nf[mu]), flip(v[c].y, nf[mu]));
+                }
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
-                    for (int b = 0; b < 3; ++b) cmad(acc[a], __ldg(w + (long)(a * 3 + b) * Vh), v[b]);
+                    for (int b = 0; b < 3; ++b) cmad(acc[a], u[a * 3 + b], v[b]);
             }
             {   // backward hop: - W_mu(x-mu)^dag in(x-mu), link based at x-mu (parity 1-par)
-                const double2 *__restrict__ w = p.W + ((long)((1 - par) * 4 + mu) * 9) * Vh + hm[mu];
-                double2 v[3];
+                const double2 *__restrict__ w = p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu];
+                double2 u[9], v[3];
+#pragma unroll
+                for (int i = 0; i < NW; ++i) u[i] = __ldg(w + (long)i * Vh);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hm[mu]);
+                if (ROWS == 2) {
+                    third_row(u);
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) v[c] = make_double2(flip(v[c].x, nb[mu]), flip(v[c].y, nb[mu]));
+                }
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
-                    for (int b = 0; b < 3; ++b)
-                        cmsub_conj(acc[a], __ldg(w + (long)(b * 3 + a) * Vh), v[b]);
+                    for (int b = 0; b < 3; ++b) cmsub_conj(acc[a], u[b * 3 + a], v[b]);
             }
+        }
+        if (ROWS == 2) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) acc[c] = make_double2(0.5 * acc[c].x, 0.5 * acc[c].y);
         }
         if (XPAY) {
             const double coeff = p.coeff_from_state ? p.mass2 + p.st->sigma0 : p.coeff;
@@ -122,12 +183,21 @@ int dslash_grid_blocks(const Geom &g) { return (g.Vh + kBlock - 1) / kBlock; }
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
 {
     const int blocks = dslash_grid_blocks(g);
-    if (p.src == nullptr)
-        launch_kernel(dslash_kernel<false, false>, blocks, kBlock, L.s, L.pdl, g, p);
-    else if (p.dot_mode == 0)
-        launch_kernel(dslash_kernel<true, false>, blocks, kBlock, L.s, L.pdl, g, p);
-    else
-        launch_kernel(dslash_kernel<true, true>, blocks, kBlock, L.s, L.pdl, g, p);
+    if (p.link_rows == 2) {
+        if (p.src == nullptr)
+            launch_kernel(dslash_kernel<false, false, 2>, blocks, kBlock, L.s, L.pdl, g, p);
+        else if (p.dot_mode == 0)
+            launch_kernel(dslash_kernel<true, false, 2>, blocks, kBlock, L.s, L.pdl, g, p);
+        else
+            launch_kernel(dslash_kernel<true, true, 2>, blocks, kBlock, L.s, L.pdl, g, p);
+    } else {
+        if (p.src == nullptr)
+            launch_kernel(dslash_kernel<false, false, 3>, blocks, kBlock, L.s, L.pdl, g, p);
+        else if (p.dot_mode == 0)
+            launch_kernel(dslash_kernel<true, false, 3>, blocks, kBlock, L.s, L.pdl, g, p);
+        else
+            launch_kernel(dslash_kernel<true, true, 3>, blocks, kBlock, L.s, L.pdl, g, p);
+    }
     return 1;
 }
 

@@ -4,6 +4,8 @@
 //   parity vector  double2 v[3][Vh]               colour-major planes, site-fastest ("ap(V,3)")
 //   links          double2 W[2][4][9][Vh]         [parity of the link's base site][mu][row*3+col][h]
 //                  W_mu(x) = 1/2 eta_mu(x) s+_mu(x) U_mu(x)   (phases absorbed)
+//   links, 2-row   double2 W[2][4][6][Vh]         rows 0 and 1 of the plain U_mu(x);
+//                  the third row, eta, the seam sign and the 1/2 are applied inside the stencil
 //   half index     h = ((t*Nz + z)*Ny + y)*(Nx/2) + x/2   == canonical address l >> 1
 // so that (D psi)(x) = sum_mu [ W_mu(x) psi(x+mu) - W_mu(x-mu)^dag psi(x-mu) ].
 #pragma once
@@ -96,12 +98,13 @@ struct Launch {
     bool pdl;
 };
 
-int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, Launch L);
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, Launch L);
 int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L);
 int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L);
 
 struct DslashParams {
     const double2 *W;
+    int link_rows;             // 3: W[2][4][9][Vh] with signs folded in; 2: W[2][4][6][Vh] plain rows 0,1
     const double2 *in;
     double2 *out;
     int out_parity;

@@ -12,7 +12,10 @@ namespace {
 
 constexpr int kBlock = 256;
 
-// one thread per (half index h, parity of the base site): 4 links each
+// one thread per (half index h, parity of the base site): 4 links each.
+// ROWS == 3: all nine entries with 1/2 eta s+ folded in.  ROWS == 2: rows 0 and 1 of the plain U,
+// bit for bit ("stores and moves only two rows"); dslash.cu rebuilds the rest.
+template <int ROWS>
 __global__ void __launch_bounds__(kBlock)
 ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__ W)
 {
@@ -36,10 +39,11 @@ ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__
     for (int mu = 0; mu < 4; ++mu) {
         double f = 0.5 * eta[mu];
         if (mu == 3 && t == (uint32_t)g.Nt - 1) f = -f;   // s+ across the t seam (C5)
+        if (ROWS == 2) f = 1.0;
         const double2 *u = U + (l * 4 + mu) * 9;
-        double2 *w = W + ((long)(par * 4 + mu) * 9) * Vh + h;
+        double2 *w = W + ((long)(par * 4 + mu) * (3 * ROWS)) * Vh + h;
 #pragma unroll
-        for (int c = 0; c < 9; ++c) {
+        for (int c = 0; c < 3 * ROWS; ++c) {
             double2 v = u[c];
             w[(long)c * Vh] = make_double2(f * v.x, f * v.y);
         }
@@ -71,10 +75,13 @@ unpack_kernel(int Vh, const double2 *__restrict__ v, double2 *__restrict__ canon
 
 }  // namespace
 
-int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, Launch L)
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, Launch L)
 {
     int blocks = (2 * g.Vh + kBlock - 1) / kBlock;
-    launch_kernel(ingest_links_kernel, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W);
+    if (link_rows == 2)
+        launch_kernel(ingest_links_kernel<2>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W);
+    else
+        launch_kernel(ingest_links_kernel<3>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W);
     return 1;
 }
 

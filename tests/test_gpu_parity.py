@@ -35,11 +35,13 @@ def q():
 class Rig:
     """One lattice: oracle + CUDA context fed the same canonical arrays."""
 
-    def __init__(self, torch, q, dims, mass, links):
+    def __init__(self, torch, q, dims, mass, links, link_rows=3):
         self.torch, self.q = torch, q
         self.dims, self.mass = dims, mass
         self.lat = oracle.Lattice(dims, links)
         self.ctx = q.Context(dims, mass)
+        if link_rows != 3:
+            self.ctx.set_option(q.QCD_OPT_LINK_ROWS, link_rows)
         self.d_links = torch.from_numpy(links).cuda()
         self.ctx.load_gauge(self.d_links)
         self.nh = self.lat.volume // 2
@@ -77,8 +79,8 @@ class Rig:
         return dict(status=st, iterations=it, true_res=tr, x=x, y=self.to_canonical(parity, d_y))
 
 
-def make_rig(torch, q, dims, kind, mass, seed, eps=0.3):
-    return Rig(torch, q, dims, mass, li.make_links(dims, kind, seed, eps))
+def make_rig(torch, q, dims, kind, mass, seed, eps=0.3, link_rows=3):
+    return Rig(torch, q, dims, mass, li.make_links(dims, kind, seed, eps), link_rows)
 
 
 # ------------------------------------------------------------------ layout
@@ -138,6 +140,57 @@ def test_set_mass_changes_mdagm(torch, q):
     assert rel_l2(rig.mdagm(E, v), rig.lat.mdagm(0.25, E, v)) <= TOL_OP
 
 
+# ------------------------------------------------------------------ two-row link storage (NEXT-1)
+
+@pytest.mark.parametrize("dims,kind", SHAPES)
+def test_two_row_dslash_and_mdagm_match_oracle(torch, q, dims, kind):
+    """QCD_OPT_LINK_ROWS = 2: same operator, third row rebuilt in the kernel; the
+    oracle is the plain definition on reconstruct_links_2row(compress_links_2row(U))."""
+    links = li.make_links(dims, kind, sum(dims), 0.3)
+    rec = oracle.reconstruct_links_2row(oracle.compress_links_2row(links))
+    rig = Rig(torch, q, dims, 0.07, links, link_rows=2)
+    lat2 = oracle.Lattice(dims, rec)
+    ve = li.make_source(dims, 41, E)
+    vo = li.make_source(dims, 42, O)
+    for lat in (lat2, rig.lat):       # the reconstructed field and the original agree to rounding
+        assert rel_l2(rig.dslash(O, ve), lat.dslash(O, ve)) <= TOL_OP
+        assert rel_l2(rig.dslash(E, vo), lat.dslash(E, vo)) <= TOL_OP
+        assert rel_l2(rig.mdagm(E, ve), lat.mdagm(0.07, E, ve)) <= TOL_OP
+        assert rel_l2(rig.mdagm(O, vo), lat.mdagm(0.07, O, vo)) <= TOL_OP
+
+
+def test_two_row_ignores_the_stored_third_row(torch, q):
+    """Only rows 0 and 1 are read: garbage in row 2 of the input changes nothing."""
+    dims = (4, 6, 4, 4)
+    links = li.make_links(dims, "random", 21)
+    bad = links.reshape(-1, 4, 3, 3, 2).copy()
+    bad[:, :, 2] = 7.25
+    a = Rig(torch, q, dims, 0.1, links, link_rows=2)
+    b = Rig(torch, q, dims, 0.1, bad.reshape(links.shape), link_rows=2)
+    v = li.make_source(dims, 3, E)
+    assert np.array_equal(a.dslash(O, v), b.dslash(O, v))
+    assert rel_l2(b.dslash(O, v), a.lat.dslash(O, v)) <= TOL_OP
+
+
+def test_two_row_option_is_per_load_and_validated(torch, q):
+    dims = (4, 4, 4, 4)
+    links = li.make_links(dims, "random", 1)
+    rig = Rig(torch, q, dims, 0.1, links)
+    v = li.make_source(dims, 1, E)
+    three = rig.dslash(O, v)
+    rig.ctx.set_option(q.QCD_OPT_LINK_ROWS, 2)      # takes effect at the next load only
+    assert np.array_equal(rig.dslash(O, v), three)
+    rig.ctx.load_gauge(rig.d_links)
+    two = rig.dslash(O, v)
+    assert rel_l2(two, three) <= 1e-14
+    rig.ctx.set_option(q.QCD_OPT_LINK_ROWS, 3)
+    rig.ctx.load_gauge(rig.d_links)
+    assert np.array_equal(rig.dslash(O, v), three)
+    for bad in (1, 4, 0):
+        with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+            rig.ctx.set_option(q.QCD_OPT_LINK_ROWS, bad)
+
+
 # ------------------------------------------------------------------ multishift CG
 
 def check_solve(rig, cfg, b, shifts, res, out, exact=None):
@@ -167,6 +220,15 @@ def test_multishift_cg_configs_1_2(torch, q, number):
     check_solve(rig, cfg, b, shifts, res, out, exact)
     ref = rig.lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, want_x=False)
     assert abs(out["iterations"] - ref["iterations"]) <= max(2, ref["iterations"] // 50)
+
+
+@pytest.mark.parametrize("number", [1, 2])
+def test_two_row_multishift_cg_configs_1_2(torch, q, number):
+    cfg, links, b, shifts, res = li.make_config_inputs(number)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links, link_rows=2)
+    out = rig.solve(cfg.parity, b, shifts, res, cfg.tol)
+    exact = rig.lat.solve_exact(cfg.mass, cfg.parity, b, shifts, res, cfg.tol)
+    check_solve(rig, cfg, b, shifts, res, out, exact)
 
 
 def test_multishift_cg_is_deterministic(torch, q):
@@ -301,6 +363,21 @@ def test_config3_full_size(torch, q):
     out = rig.solve(E, b, shifts, res, cfg.tol)
     exact = rig.lat.solve_exact(cfg.mass, E, b, shifts, res, cfg.tol)
     check_solve(rig, cfg, b, shifts, res, out, exact)
+
+
+@pytest.mark.slow
+def test_config3_full_size_two_row(torch, q):
+    cfg, links, b, shifts, res = li.make_config_inputs(3)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links, link_rows=2)
+    vo = li.make_source(cfg.dims, 43, O)
+    assert rel_l2(rig.dslash(O, b), rig.lat.dslash(O, b)) <= TOL_OP
+    assert rel_l2(rig.dslash(E, vo), rig.lat.dslash(E, vo)) <= TOL_OP
+    assert rel_l2(rig.mdagm(E, b), rig.lat.mdagm(cfg.mass, E, b)) <= TOL_OP
+    out = rig.solve(E, b, shifts, res, cfg.tol)
+    assert out["status"] == 0 and (out["true_res"] <= 1.5 * cfg.tol).all()
+    for k in (0, 11):
+        xs, _, tr, st = rig.lat.cg(cfg.mass, E, shifts[k], b, 1e-14, max_iter=5000)
+        assert st == 0 and rel_l2(out["x"][k], xs) <= TOL_X
 
 
 def _sampled_shift_check(rig, cfg, b, shifts, out, ks):
