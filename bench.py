@@ -214,6 +214,7 @@ def main():
     ap.add_argument("--link-rows", type=int, default=3, choices=[2, 3],
                     help="QCD_OPT_LINK_ROWS for the whole run (default 3, the paper's uncompressed "
                          "storage; the default run also reports a two-row section)")
+    ap.add_argument("--tgroup", type=int, default=0, help="QCD_OPT_TGROUP (0 = library default)")
     ap.add_argument("--no-two-row", action="store_true", help="skip the extra two-row section")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
@@ -252,6 +253,8 @@ def main():
     if args.cg_batch:
         ctx.set_option(q.QCD_OPT_CG_BATCH, args.cg_batch)
     ctx.set_option(q.QCD_OPT_LINK_ROWS, args.link_rows)
+    if args.tgroup:
+        ctx.set_option(q.QCD_OPT_TGROUP, args.tgroup)
     d_links = torch.from_numpy(links).cuda()
     ctx.load_gauge(d_links)
     torch.cuda.synchronize()
@@ -406,6 +409,22 @@ def main():
         e2e["gauge_ingest_s"] = time.perf_counter() - w0
         e2e["gauge_h2d_bytes"] = links.nbytes
         line["e2e"] = e2e
+
+        if not args.no_solve:
+            # the paper's step 2, (M^dag M)^(-1/2) phi via eq. 8
+            xmin, xmax = 0.9 * cfg.mass ** 2, 8.5      # the paper's xmax = 34 in its normalisation
+            ts = []
+            for _ in range(3):
+                torch.cuda.synchronize()
+                w0 = time.perf_counter()
+                st, it, tr, delta = ctx.inv_sqrt(cfg.parity, d_b, cfg.nshift, xmin, xmax, cfg.tol,
+                                                 100000, d_y)
+                ts.append(time.perf_counter() - w0)
+                assert st == 0 and tr.max() <= 1.5 * cfg.tol, (st, tr)
+            line["inv_sqrt"] = {"n": cfg.nshift, "xmin": xmin, "xmax": xmax, "delta": delta,
+                                "iterations": it, "s_per_apply": statistics.median(ts[1:]),
+                                "what": "qcd_inv_sqrt: Zolotarev coefficients + one multishift CG + "
+                                        "fused c0*phi + sum c_k x_k"}
 
         if R == 3 and not args.no_two_row:
             # the same sections A and C with two-row link storage

@@ -70,7 +70,7 @@ QCD_API qcd_status qcd_destroy(qcd_ctx *ctx);
 QCD_API qcd_status qcd_set_mass(qcd_ctx *ctx, double mass);
 QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 
-/* Execution options.  The first three do not change a single bit of any result.
+/* Execution options.  All but QCD_OPT_LINK_ROWS leave every result bit-identical.
  *   QCD_OPT_PDL       (default 1) launch every kernel with programmatic dependent launch, so that its
  *                     index arithmetic overlaps the tail of its predecessor in the stream or graph.
  *   QCD_OPT_CG_GRAPH  (default 1) qcd_multishift_cg replays one captured CUDA graph per batch of
@@ -78,6 +78,11 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *   QCD_OPT_CG_BATCH  (default 8) iterations per batch; the host reads the device's convergence flag
  *                     once per batch, one batch late, so up to 2 batches of early-exit kernels follow
  *                     convergence.  1 <= value <= 1024.
+ *   QCD_OPT_TGROUP    (default 0 = chosen by the library) order in which the Dslash CTAs walk the
+ *                     lattice: groups of this many 128-site chunks of a t-slice are processed for all t
+ *                     before the next group starts, so +-t neighbours are reused out of L2.  Does not
+ *                     change a single bit of any result.  Values above the chunks per slice mean plain
+ *                     lexicographic order.
  *   QCD_OPT_LINK_ROWS (default 3) how the NEXT qcd_load_gauge stores the links.  3: all nine entries
  *                     (576 V bytes, "72V double precision words").  2: two-row storage
  *                     (384 V bytes): "one often stores and moves only two rows ... of the (3 x 3)
@@ -86,7 +91,7 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     SU(3) (unitary, det = 1): rows 2 of the input are ignored.  Results differ from
  *                     the 3-row path at rounding level only (relative 1e-15) for SU(3) input.
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
-enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3 };
+enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */
@@ -127,6 +132,29 @@ QCD_API qcd_status qcd_multishift_cg(qcd_ctx *ctx, int parity, const double *d_b
                              const double *shifts, const double *residues, double tol,
                              int max_iter, double *d_x, double *d_y, int *iterations,
                              double *true_res);
+
+/* the paper's "step 2", (M^dag M)^(-1/2) phi, through the rational
+ * approximation of eq. 8:  x^(-1/2) ~= c_0 + sum_{k<n} c_k / (x + d_k).
+ *
+ * qcd_inv_sqrt_coeffs: HOST ONLY, needs no context and no GPU.  Writes the minimax (relative error)
+ * approximation of type (n, n) on [xmin, xmax] -- what the paper takes from Mathematica's MiniMax
+ * (appendix :288-304), computed here from Zolotarev's closed form in double precision:
+ *   c0       host, 1 double;   coef, shift: host, n doubles each (c_k > 0; d_k > 0, ascending)
+ *   delta    host, may be NULL: max over [xmin, xmax] of |1 - sqrt(x) r(x)|
+ * The caller chooses xmin < lambda_min(M^dag M) (>= m^2 in this normalisation) and
+ * xmax > lambda_max (m^2 + 4 for unit links, about 7 for random SU(3), never above m^2 + 16; the
+ * paper keeps xmax = 34 in its normalisation, which is 8.5 here).  QCD_EINVAL unless 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax.
+ *
+ * qcd_inv_sqrt: d_out = c_0 d_phi + sum_k c_k (M^dag M + d_k)^(-1) d_phi on `parity` with those
+ * coefficients, by ONE multishift CG (n shifts) and a fused combine.  Arguments as
+ * qcd_multishift_cg; true_res has n entries (shift order ascending); d_out must not alias d_phi.
+ * The result differs from (M^dag M)^(-1/2) phi by at most delta (approximation) + O(tol) (solver)
+ * in relative 2-norm, provided the spectrum lies in [xmin, xmax].  Synchronises. */
+QCD_API qcd_status qcd_inv_sqrt_coeffs(int n, double xmin, double xmax, double *c0, double *coef,
+                                       double *shift, double *delta);
+QCD_API qcd_status qcd_inv_sqrt(qcd_ctx *ctx, int parity, const double *d_phi, int n, double xmin,
+                                double xmax, double tol, int max_iter, double *d_out,
+                                int *iterations, double *true_res, double *delta);
 
 /* Host-buffer forms (canonical layout on the host; H2D copy, pack, compute, unpack, D2H copy and a
  * stream synchronise all happen inside the call).  h_x: nshift canonical parity vectors or NULL;

@@ -15,7 +15,7 @@ import re
 import numpy as np
 
 QCD_EVEN, QCD_ODD = 0, 1
-QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH, QCD_OPT_LINK_ROWS = 0, 1, 2, 3
+QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH, QCD_OPT_LINK_ROWS, QCD_OPT_TGROUP = 0, 1, 2, 3, 4
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONV, QCD_ESTATE = range(6)
 _STATUS_NAMES = ["QCD_OK", "QCD_EINVAL", "QCD_ENOMEM", "QCD_ECUDA", "QCD_ENOTCONV", "QCD_ESTATE"]
 
@@ -40,6 +40,8 @@ _SIGNATURES = {
     "qcd_mdagm": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_multishift_cg": (_ci, [_vp, _ci, _vp, _ci, _vp, _vp, _cd, _ci, _vp, _vp,
                                 ctypes.POINTER(_ci), _vp]),
+    "qcd_inv_sqrt_coeffs": (_ci, [_ci, _cd, _cd, _vp, _vp, _vp, _vp]),
+    "qcd_inv_sqrt": (_ci, [_vp, _ci, _vp, _ci, _cd, _cd, _cd, _ci, _vp, ctypes.POINTER(_ci), _vp, _vp]),
     "qcd_dslash_host": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_mdagm_host": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_multishift_cg_host": (_ci, [_vp, _ci, _vp, _ci, _vp, _vp, _cd, _ci, _vp, _vp,
@@ -110,6 +112,18 @@ def _host_ptr(a: np.ndarray) -> int:
     if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous):
         raise TypeError("expected a C-contiguous float64 numpy array")
     return a.ctypes.data
+
+
+def inv_sqrt_coeffs(n: int, xmin: float, xmax: float):
+    """qcd_inv_sqrt_coeffs (host only): returns (c0, c[n], d[n], delta)."""
+    lib = load_library()
+    c0, delta = np.zeros(1), np.zeros(1)
+    c, d = np.zeros(max(int(n), 1)), np.zeros(max(int(n), 1))
+    st = lib.qcd_inv_sqrt_coeffs(int(n), float(xmin), float(xmax), _host_ptr(c0), _host_ptr(c),
+                                 _host_ptr(d), _host_ptr(delta))
+    if st != QCD_OK:
+        raise QcdError(st, "qcd_inv_sqrt_coeffs", lib.qcd_last_error(None).decode())
+    return float(c0[0]), c, d, float(delta[0])
 
 
 class Context:
@@ -193,6 +207,18 @@ class Context:
             None if d_y is None else _dev_ptr(d_y), ctypes.byref(it), _host_ptr(true_res))
         self._check(st, "qcd_multishift_cg", allow=(QCD_ENOTCONV,))
         return st, it.value, true_res
+
+    def inv_sqrt(self, parity: int, d_phi, n: int, xmin: float, xmax: float, tol: float,
+                 max_iter: int, d_out):
+        """Returns (status, iterations, true_res[n], delta)."""
+        true_res = np.full(int(n), np.nan)
+        delta = np.zeros(1)
+        it = _ci(0)
+        st = self._lib.qcd_inv_sqrt(self._h, parity, _dev_ptr(d_phi), int(n), float(xmin), float(xmax),
+                                    float(tol), int(max_iter), _dev_ptr(d_out), ctypes.byref(it),
+                                    _host_ptr(true_res), _host_ptr(delta))
+        self._check(st, "qcd_inv_sqrt", allow=(QCD_ENOTCONV,))
+        return st, it.value, true_res, float(delta[0])
 
     # -- host entry points (canonical numpy arrays; copies happen inside the C call) --
     def load_gauge_host(self, h_links: np.ndarray):

@@ -87,6 +87,12 @@ qcd_status check_launch(qcd_ctx *c, const char *what)
     return QCD_OK;
 }
 
+// Dslash CTA order (dslash.cu).  Plain lexicographic order is best while one t-slice of CTAs moves
+// less link data than L2 can hold behind it (measured on B200: 121.6 us plain vs 122.4-126 grouped at
+// 48^3x12, 432 chunks = 69 MB per slice); beyond that the +-t reuse falls out of L2 and groups of 256
+// chunks win (64^3x16, 1024 chunks = 163 MB per slice: 380 us vs 398 plain).
+int auto_tgroup(const Geom &g) { return g.chunks >= 640 ? 256 : g.chunks; }
+
 bool bad_parity(int p) { return p != QCD_EVEN && p != QCD_ODD; }
 
 qcd_status ensure_host_staging(qcd_ctx *c)
@@ -213,6 +219,8 @@ qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx
     g.Vh = (int)(V / 2);
     g.sy = g.Nxh; g.sz = g.Nxh * g.Ny; g.st = g.Nxh * g.Ny * g.Nz;
     g.dxh.init(g.Nxh); g.dy.init(g.Ny); g.dz.init(g.Nz);
+    g.chunks = dslash_chunks(g);
+    g.tgroup = auto_tgroup(g);
     c->n2 = 3L * g.Vh;
     c->vec_bytes = (size_t)c->n2 * sizeof(double2);
 
@@ -278,6 +286,11 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
     case QCD_OPT_CG_BATCH:
         if (value < 1 || value > 1024) return fail(c, QCD_EINVAL, "qcd_set_option: batch must be in [1, 1024]");
         c->opt_cg_batch = (int)value;
+        return QCD_OK;
+    case QCD_OPT_TGROUP:
+        if (value < 0) return fail(c, QCD_EINVAL, "qcd_set_option: tgroup must be >= 0");
+        c->g.tgroup = value == 0 ? auto_tgroup(c->g) : value > c->g.chunks ? c->g.chunks : (int)value;
+        if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }   // Geom is baked in
         return QCD_OK;
     case QCD_OPT_LINK_ROWS:
         if (value != 2 && value != 3) return fail(c, QCD_EINVAL, "qcd_set_option: link rows must be 2 or 3");
@@ -354,10 +367,15 @@ qcd_status qcd_mdagm(qcd_ctx *c, int parity, const double *d_in, double *d_out)
     return check_launch(c, "qcd_mdagm");
 }
 
-qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshift,
-                             const double *shifts, const double *residues, double tol,
-                             int max_iter, double *d_x, double *d_y, int *iterations,
-                             double *true_res)
+}  // extern "C"
+
+namespace {
+
+// qcd_multishift_cg with the optional c_0 term of eq. 8: y = c0 b + sum_k residues[k] x_k
+qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nshift,
+                              const double *shifts, const double *residues, double tol,
+                              int max_iter, double *d_x, double *d_y, int *iterations,
+                              double *true_res, bool with_c0, double c0)
 {
     if (!c) return QCD_EINVAL;
     if (bad_parity(parity) || !d_b || !shifts || !residues || !iterations || !true_res)
@@ -437,7 +455,8 @@ qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshi
                                             c->results + order[k], c->L());
     }
     if (d_y)
-        c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, (double2 *)d_y, c->L());
+        c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, c0,
+                                      with_c0 ? b : nullptr, (double2 *)d_y, c->L());
     s = check_launch(c, "qcd_multishift_cg");
     if (s != QCD_OK) return s;
     QCD_CUDA(c, cudaMemcpyAsync(c->h_results, c->results, nshift * sizeof(double), cudaMemcpyDeviceToHost, st));
@@ -451,6 +470,43 @@ qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshi
     const bool converged = rho_b == 0.0 || std::sqrt(h.rho / rho_b) <= tol;
     if (!converged) return fail(c, QCD_ENOTCONV, "qcd_multishift_cg: max_iter reached");
     return QCD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshift,
+                             const double *shifts, const double *residues, double tol,
+                             int max_iter, double *d_x, double *d_y, int *iterations,
+                             double *true_res)
+{
+    return multishift_cg_impl(c, parity, d_b, nshift, shifts, residues, tol, max_iter, d_x, d_y,
+                              iterations, true_res, false, 0.0);
+}
+
+qcd_status qcd_inv_sqrt_coeffs(int n, double xmin, double xmax, double *c0, double *coef,
+                               double *shift, double *delta)
+{
+    if (!c0 || !coef || !shift)
+        return fail(nullptr, QCD_EINVAL, "qcd_inv_sqrt_coeffs: NULL output");
+    if (zolotarev_inv_sqrt(n, xmin, xmax, c0, coef, shift, delta) != 0)
+        return fail(nullptr, QCD_EINVAL,
+                    "qcd_inv_sqrt_coeffs: need 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax");
+    return QCD_OK;
+}
+
+qcd_status qcd_inv_sqrt(qcd_ctx *c, int parity, const double *d_phi, int n, double xmin,
+                        double xmax, double tol, int max_iter, double *d_out, int *iterations,
+                        double *true_res, double *delta)
+{
+    if (!c) return QCD_EINVAL;
+    if (!d_out || d_out == d_phi) return fail(c, QCD_EINVAL, "qcd_inv_sqrt: bad output pointer");
+    double c0, coef[kMaxShifts], shift[kMaxShifts];
+    if (zolotarev_inv_sqrt(n, xmin, xmax, &c0, coef, shift, delta) != 0)
+        return fail(c, QCD_EINVAL, "qcd_inv_sqrt: need 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax");
+    return multishift_cg_impl(c, parity, d_phi, n, shift, coef, tol, max_iter, nullptr, d_out,
+                              iterations, true_res, true, c0);
 }
 
 qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, double *h_out)

@@ -149,14 +149,19 @@ struct CombineArgs {
     int n;
 };
 
-// y = sum_k c_k x_k   (eq. 8 without c_0)
+// y = c_0 b + sum_k c_k x_k   (eq. 8; b == nullptr: without the c_0 term)
 __global__ void __launch_bounds__(kBlock)
-combine_kernel(long n2, const double2 *__restrict__ x, const CombineArgs a, double2 *__restrict__ y)
+combine_kernel(long n2, const double2 *__restrict__ x, const CombineArgs a, double c0,
+               const double2 *__restrict__ b, double2 *__restrict__ y)
 {
     pdl_wait();
     pdl_launch_dependents();
     for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
         double2 s = make_double2(0.0, 0.0);
+        if (b != nullptr) {
+            const double2 v = __ldg(b + i);
+            s = make_double2(c0 * v.x, c0 * v.y);
+        }
 #pragma unroll 4
         for (int k = 0; k < a.n; ++k) {
             const double2 v = __ldg(x + a.xoff[k] + i);
@@ -208,12 +213,12 @@ int launch_residual_norm(long n2, const double2 *b, const double2 *q, const doub
 }
 
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
-                   int nshift, double2 *y, Launch L)
+                   int nshift, double c0, const double2 *b, double2 *y, Launch L)
 {
     CombineArgs a;
     a.n = nshift;
     for (int k = 0; k < nshift; ++k) { a.xoff[k] = xoff_host[k]; a.c[k] = residues[k]; }
-    launch_kernel(combine_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, x, a, y);
+    launch_kernel(combine_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, x, a, c0, b, y);
     return 1;
 }
 

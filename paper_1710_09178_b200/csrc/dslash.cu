@@ -15,10 +15,16 @@ namespace qcd {
 
 namespace {
 
-constexpr int kBlock = 128;
+#ifndef QCD_DSLASH_BLOCK
+#define QCD_DSLASH_BLOCK 128
+#endif
+constexpr int kBlock = QCD_DSLASH_BLOCK;
+#ifndef QCD_DSLASH3_MINB
+#define QCD_DSLASH3_MINB 4   // 128 registers: 24.4 / 120.5 / 393 us; unbounded (60 regs) 26.0 / 129 / 404; 1 (254 regs) 25.7 / 120.2 / 394
+#endif
 // minimum resident CTAs per SM asked of ptxas for the two-row kernel (caps its registers)
 #ifndef QCD_DSLASH2_MINB
-#define QCD_DSLASH2_MINB 7   // measured on B200: 7 beats 1, 6, 8 at 32^3x8 (whole grid resident in one wave)
+#define QCD_DSLASH2_MINB 4   // measured on B200 (32^3x8 / 48^3x12 / 64^3x16): 4 -> 16.8 / 83.4 / 274 us; 7 -> 17.1 / 88.6 / 276; 1 -> 18.9 / - / 296
 #endif
 
 // acc += w * v
@@ -69,22 +75,35 @@ __device__ __forceinline__ void third_row(double2 *u)
 //            here.  All of them depend on the OUTPUT site only: eta_mu does not depend on x_mu, and
 //            the seam sign of the backward hop is s-_mu(x).
 template <bool XPAY, bool DOT, int ROWS>
-__global__ void __launch_bounds__(kBlock, ROWS == 2 ? QCD_DSLASH2_MINB : 1)
+__global__ void __launch_bounds__(kBlock, ROWS == 2 ? QCD_DSLASH2_MINB : QCD_DSLASH3_MINB)
 dslash_kernel(const Geom g, const DslashParams p)
 {
     constexpr int NW = 3 * ROWS;
     const int Vh = g.Vh;
-    const uint32_t h = blockIdx.x * kBlock + threadIdx.x;
-    const bool valid = h < (uint32_t)Vh;
+    // CTA order.  A chunk is kBlock consecutive sites of one t-slice.  The chunks of a slice are cut
+    // into groups of g.tgroup; CTAs walk group by group, and inside a group t runs slowest:
+    //     blockIdx = (group * Nt + t) * tgroup + chunk_in_group        (last group may be shorter)
+    // so the CTAs that read the same input sites as +-t neighbours are tgroup CTAs apart instead of a
+    // whole t-slice of CTAs (1024 CTAs = 163 MB of link traffic at 64^3x16, more than L2 holds: ncu
+    // showed 2.7-2.8 GB of DRAM reads per apply against 2.52 GB algorithmic), while each group still
+    // streams tgroup * 2 KB contiguous bytes of every link plane.  tgroup == chunks: plain h order.
+    const uint32_t per_group = (uint32_t)g.tgroup * (uint32_t)g.Nt;
+    const uint32_t grp = blockIdx.x / per_group, rem = blockIdx.x - grp * per_group;
+    const uint32_t first = grp * (uint32_t)g.tgroup;
+    const uint32_t width = min((uint32_t)g.tgroup, (uint32_t)g.chunks - first);   // chunks in this group
+    const uint32_t t = rem / width;
+    const uint32_t chunk = first + (rem - t * width);
+    const uint32_t sl = chunk * kBlock + threadIdx.x;          // index inside the t-slice
+    const bool valid = sl < (uint32_t)g.st;
+    const uint32_t h = t * (uint32_t)g.st + sl;
     double dot = 0.0;
     const int par = p.out_parity;
     int hp[4], hm[4];   // half indices of the 8 neighbours (all of the opposite parity)
     int nf[4] = {0, 0, 0, 0}, nb[4] = {0, 0, 0, 0};   // ROWS == 2: 1 where the hop carries a minus sign
     if (valid) {
-        uint32_t q, xh, y, z, t;
-        g.dxh.divmod(h, q, xh);
-        g.dy.divmod(q, q, y);
-        g.dz.divmod(q, t, z);
+        uint32_t q, xh, y, z;
+        g.dxh.divmod(sl, q, xh);
+        g.dy.divmod(q, z, y);
         const int r = (y + z + t + par) & 1;      // x = 2*xh + r
         {
             const int xh_p = r ? ((int)xh + 1 == g.Nxh ? 0 : (int)xh + 1) : (int)xh;
@@ -178,7 +197,8 @@ dslash_kernel(const Geom g, const DslashParams p)
 
 }  // namespace
 
-int dslash_grid_blocks(const Geom &g) { return (g.Vh + kBlock - 1) / kBlock; }
+int dslash_chunks(const Geom &g) { return (g.st + kBlock - 1) / kBlock; }
+int dslash_grid_blocks(const Geom &g) { return dslash_chunks(g) * g.Nt; }
 
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
 {

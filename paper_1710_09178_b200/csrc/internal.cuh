@@ -40,6 +40,8 @@ struct Geom {
     int Vh;          // sites of one parity
     int sy, sz, st;  // half-index strides of +y, +z, +t
     FastDiv dxh, dy, dz;
+    int chunks;      // Dslash CTAs per t-slice
+    int tgroup;      // chunks per group of the Dslash CTA order (dslash.cu), 1 <= tgroup <= chunks
 };
 
 // Device-resident scalars of the multishift CG; no host round trip per iteration.
@@ -120,6 +122,7 @@ struct DslashParams {
 };
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L);
 int dslash_grid_blocks(const Geom &g);
+int dslash_chunks(const Geom &g);
 
 // BLAS-1 (n2 = 3*Vh double2 elements per vector)
 int blas_grid_blocks(long n2);
@@ -132,7 +135,11 @@ int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, l
 // scratch = || b - (q + sigma x) ||^2   and  scratch = ||b||^2
 int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
                          double *partial, CgState *st, double *result, Launch L);
+// y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
-                   int nshift, double2 *y, Launch L);
+                   int nshift, double c0, const double2 *b, double2 *y, Launch L);
+
+// host only (zolotarev.cu): minimax x^(-1/2) ~= c0 + sum_k c[k]/(x + d[k]) on [xmin, xmax]; 0 = ok
+int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, double *d, double *delta);
 
 }  // namespace qcd

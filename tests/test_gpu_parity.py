@@ -67,6 +67,11 @@ class Rig:
         self.ctx.mdagm(parity, self.to_internal(parity, v), d_out)
         return self.to_canonical(parity, d_out)
 
+    def mdagm_internal(self, parity, d_in):
+        d_out = self.ctx.new_vector()
+        self.ctx.mdagm(parity, d_in, d_out)
+        return self.to_canonical(parity, d_out)
+
     def solve(self, parity, b, shifts, residues, tol, max_iter=100000, own_x=True):
         n = len(shifts)
         d_x = self.ctx.new_vector(n) if own_x else None
@@ -261,6 +266,27 @@ def test_execution_options_do_not_change_a_single_bit(torch, q):
         rig.ctx.set_option(99, 1)
 
 
+def test_cta_order_option_does_not_change_a_single_bit(torch, q):
+    """QCD_OPT_TGROUP only permutes which CTA handles which 128-site chunk (3 ragged chunks per
+    t-slice here); the CG reduction order is by blockIdx, so only Dslash/M^dag M must be bit-equal,
+    the solve to rounding."""
+    dims, mass = (12, 6, 10, 4), 0.07
+    rig = make_rig(torch, q, dims, "random", mass, 9)
+    ve, vo = li.make_source(dims, 1, E), li.make_source(dims, 2, O)
+    ref = (rig.dslash(O, ve), rig.dslash(E, vo), rig.mdagm(E, ve))
+    shifts, res = np.array([0.01, 0.3, 1.5]), np.ones(3)
+    sref = rig.solve(E, ve, shifts, res, 1e-10)
+    for g in (1, 2, 3, 100000, 0):
+        rig.ctx.set_option(q.QCD_OPT_TGROUP, g)
+        out = (rig.dslash(O, ve), rig.dslash(E, vo), rig.mdagm(E, ve))
+        assert all(np.array_equal(a, b) for a, b in zip(out, ref))
+        s = rig.solve(E, ve, shifts, res, 1e-10)
+        assert s["status"] == 0 and rel_l2(s["x"], sref["x"]) <= 1e-12
+    assert rel_l2(ref[0], rig.lat.dslash(O, ve)) <= TOL_OP
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.ctx.set_option(q.QCD_OPT_TGROUP, -1)
+
+
 def test_multishift_cg_odd_parity_unsorted_shifts_zero_shift(torch, q):
     dims, mass = (4, 6, 4, 4), 0.08
     rig = make_rig(torch, q, dims, "random", mass, 7)
@@ -346,6 +372,50 @@ def test_host_entry_points_equal_device_entry_points(torch, q):
     assert st == 0 and it == dev["iterations"]
     assert np.array_equal(hx, dev["x"]) and np.array_equal(hy, dev["y"])
     assert np.array_equal(tr, dev["true_res"])
+
+
+# ------------------------------------------------------------------ (M^dag M)^(-1/2) phi  (NEXT-2)
+
+@pytest.mark.parametrize("number,n", [(1, 10), (2, 12)])
+def test_inv_sqrt_matches_oracle_and_dense_definition(torch, q, number, n):
+    """qcd_inv_sqrt against (i) the oracle's eq. 8 with the ORACLE's coefficients and polished
+    solves, (ii) the definition Q diag(lambda^-1/2) Q^dag phi through eigh (config 1 only)."""
+    from oracle import rational as R
+    from helpers import c as cplx, dense_from_operator
+    cfg, links, b, _, _ = li.make_config_inputs(number)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    xmin, xmax = 0.9 * cfg.mass ** 2, 8.5      # the paper's xmax = 34 in its normalisation (PAPER.md:292)
+    d_out = rig.ctx.new_vector()
+    st, it, tr, delta = rig.ctx.inv_sqrt(E, rig.to_internal(E, b), n, xmin, xmax, 1e-11, 100000, d_out)
+    got = rig.to_canonical(E, d_out)
+    z = R.zolotarev_inv_sqrt(n, xmin, xmax)
+    assert st == 0 and (tr <= 1.5e-11).all() and abs(delta - z["delta"]) <= 1e-6 * z["delta"]
+    sol = rig.lat.solve_exact(cfg.mass, E, b, z["d"], z["c"], 1e-11)
+    assert rel_l2(got, z["c0"] * b + sol["y"]) <= TOL_X
+    if number == 1:
+        a = dense_from_operator(lambda v: rig.lat.mdagm(cfg.mass, E, v), rig.nh)
+        lam, qm = np.linalg.eigh(a)
+        assert xmin < lam.min() and lam.max() < xmax
+        phi = cplx(b).reshape(-1)
+        exact = qm @ ((qm.conj().T @ phi) / np.sqrt(lam))
+        err = np.linalg.norm(cplx(got).reshape(-1) - exact) / np.linalg.norm(exact)
+        assert err <= 1.05 * delta + 1e-9
+        # applying it twice inverts M^dag M:  A r(A)^2 phi = phi +- 2 delta
+        d_2 = rig.ctx.new_vector()
+        rig.ctx.inv_sqrt(E, d_out, n, xmin, xmax, 1e-11, 100000, d_2)
+        back = rig.mdagm_internal(E, d_2)
+        assert rel_l2(back, b) <= 2.2 * delta + 1e-8
+
+
+def test_inv_sqrt_argument_errors(torch, q):
+    rig = make_rig(torch, q, (4, 4, 4, 4), "random", 0.1, 1)
+    v, w = rig.ctx.new_vector(), rig.ctx.new_vector()
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.ctx.inv_sqrt(E, v, 0, 0.01, 5.0, 1e-10, 100, w)
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.ctx.inv_sqrt(E, v, 4, 5.0, 0.01, 1e-10, 100, w)
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.ctx.inv_sqrt(E, v, 4, 0.01, 5.0, 1e-10, 100, v)
 
 
 # ------------------------------------------------------------------ full-size configs 3, 4, 5
