@@ -70,7 +70,7 @@ QCD_API qcd_status qcd_destroy(qcd_ctx *ctx);
 QCD_API qcd_status qcd_set_mass(qcd_ctx *ctx, double mass);
 QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 
-/* Execution options.  All but QCD_OPT_LINK_ROWS leave every result bit-identical.
+/* Execution options.  PDL, CG_GRAPH and CG_BATCH leave every result bit-identical.
  *   QCD_OPT_PDL       (default 1) launch every kernel with programmatic dependent launch, so that its
  *                     index arithmetic overlaps the tail of its predecessor in the stream or graph.
  *   QCD_OPT_CG_GRAPH  (default 1) qcd_multishift_cg replays one captured CUDA graph per batch of
@@ -80,9 +80,10 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     convergence.  1 <= value <= 1024.
  *   QCD_OPT_TGROUP    (default 0 = chosen by the library) order in which the Dslash CTAs walk the
  *                     lattice: groups of this many 128-site chunks of a t-slice are processed for all t
- *                     before the next group starts, so +-t neighbours are reused out of L2.  Does not
- *                     change a single bit of any result.  Values above the chunks per slice mean plain
- *                     lexicographic order.
+ *                     before the next group starts, so +-t neighbours are reused out of L2.  Dslash and
+ *                     M^dag M stay bit-identical; CG results change at rounding level only (the
+ *                     <p,Ap> partial sums are added in CTA order).  Values above the chunks per slice
+ *                     mean plain lexicographic order.
  *   QCD_OPT_LINK_ROWS (default 3) how the NEXT qcd_load_gauge stores the links.  3: all nine entries
  *                     (576 V bytes, "72V double precision words").  2: two-row storage
  *                     (384 V bytes): "one often stores and moves only two rows ... of the (3 x 3)
