@@ -84,6 +84,11 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     M^dag M stay bit-identical; CG results change at rounding level only (the
  *                     <p,Ap> partial sums are added in CTA order).  Values above the chunks per slice
  *                     mean plain lexicographic order.
+ *   QCD_OPT_L2_PERSIST_MB (default 0 = off) applies at the NEXT qcd_load_gauge: Dslash launches carry
+ *                     an L2 access-policy window that keeps this many MB of the gauge field in the
+ *                     persisting set-aside of L2 (capped by the device limits; the limit is device-
+ *                     wide).  Helps back-to-back applies on lattices slightly larger than L2, hurts the
+ *                     CG when the set-aside takes L2 away from its vectors.  Bit-identical results.
  *   QCD_OPT_LINK_ROWS (default 3) how the NEXT qcd_load_gauge stores the links.  3: all nine entries
  *                     (576 V bytes, "72V double precision words").  2: two-row storage
  *                     (384 V bytes): "one often stores and moves only two rows ... of the (3 x 3)
@@ -92,7 +97,8 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     SU(3) (unitary, det = 1): rows 2 of the input are ignored.  Results differ from
  *                     the 3-row path at rounding level only (relative 1e-15) for SU(3) input.
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
-enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4 };
+enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
+       QCD_OPT_L2_PERSIST_MB = 5 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

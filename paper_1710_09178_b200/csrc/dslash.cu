@@ -205,18 +205,18 @@ int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
     const int blocks = dslash_grid_blocks(g);
     if (p.link_rows == 2) {
         if (p.src == nullptr)
-            launch_kernel(dslash_kernel<false, false, 2>, blocks, kBlock, L.s, L.pdl, g, p);
+            launch_kernel_apw(dslash_kernel<false, false, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
         else if (p.dot_mode == 0)
-            launch_kernel(dslash_kernel<true, false, 2>, blocks, kBlock, L.s, L.pdl, g, p);
+            launch_kernel_apw(dslash_kernel<true, false, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
         else
-            launch_kernel(dslash_kernel<true, true, 2>, blocks, kBlock, L.s, L.pdl, g, p);
+            launch_kernel_apw(dslash_kernel<true, true, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
     } else {
         if (p.src == nullptr)
-            launch_kernel(dslash_kernel<false, false, 3>, blocks, kBlock, L.s, L.pdl, g, p);
+            launch_kernel_apw(dslash_kernel<false, false, 3>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
         else if (p.dot_mode == 0)
-            launch_kernel(dslash_kernel<true, false, 3>, blocks, kBlock, L.s, L.pdl, g, p);
+            launch_kernel_apw(dslash_kernel<true, false, 3>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
         else
-            launch_kernel(dslash_kernel<true, true, 3>, blocks, kBlock, L.s, L.pdl, g, p);
+            launch_kernel_apw(dslash_kernel<true, true, 3>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
     }
     return 1;
 }

@@ -76,21 +76,39 @@ __device__ __forceinline__ void pdl_launch_dependents()
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
+// apw != nullptr: the launch carries an L2 access-policy window (persisting lines for part of the
+// gauge field, see api.cu); as a launch attribute it is recorded in captured graph nodes too.
 template <class... KArgs, class... Args>
-inline cudaError_t launch_kernel(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s,
-                                 bool pdl, Args... args)
+inline cudaError_t launch_kernel_apw(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s,
+                                     bool pdl, const cudaAccessPolicyWindow *apw, Args... args)
 {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)block);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = s;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute attr[2];
+    unsigned n = 0;
+    if (pdl) {
+        attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[n].val.programmaticStreamSerializationAllowed = 1;
+        ++n;
+    }
+    if (apw != nullptr) {
+        attr[n].id = cudaLaunchAttributeAccessPolicyWindow;
+        attr[n].val.accessPolicyWindow = *apw;
+        ++n;
+    }
     cfg.attrs = attr;
-    cfg.numAttrs = pdl ? 1u : 0u;
+    cfg.numAttrs = n;
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+template <class... KArgs, class... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), int grid, int block, cudaStream_t s,
+                                 bool pdl, Args... args)
+{
+    return launch_kernel_apw(kernel, grid, block, s, pdl, nullptr, args...);
 }
 #endif
 
@@ -98,6 +116,7 @@ inline cudaError_t launch_kernel(void (*kernel)(KArgs...), int grid, int block, 
 struct Launch {
     cudaStream_t s;
     bool pdl;
+    const cudaAccessPolicyWindow *apw = nullptr;   // only the Dslash launches use it
 };
 
 int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, Launch L);

@@ -285,6 +285,15 @@ def test_cta_order_option_does_not_change_a_single_bit(torch, q):
     assert rel_l2(ref[0], rig.lat.dslash(O, ve)) <= TOL_OP
     with pytest.raises(q.QcdError, match="QCD_EINVAL"):
         rig.ctx.set_option(q.QCD_OPT_TGROUP, -1)
+    # L2 persisting window: applies at the next load, results unchanged
+    rig.ctx.set_option(q.QCD_OPT_TGROUP, 0)
+    rig.ctx.set_option(q.QCD_OPT_L2_PERSIST_MB, 16)
+    rig.ctx.load_gauge(rig.d_links)
+    assert np.array_equal(rig.dslash(O, ve), ref[0]) and np.array_equal(rig.mdagm(E, ve), ref[2])
+    s = rig.solve(E, ve, shifts, res, 1e-10)
+    assert s["status"] == 0 and np.array_equal(s["x"], sref["x"])
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.ctx.set_option(q.QCD_OPT_L2_PERSIST_MB, -1)
 
 
 def test_multishift_cg_odd_parity_unsorted_shifts_zero_shift(torch, q):
