@@ -257,7 +257,7 @@ qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx
     const int nblk = std::max(dslash_grid_blocks(g), blas_grid_blocks(c->n2));
     if (dev_alloc(&c->W, (size_t)72 * g.Vh) != cudaSuccess ||
         dev_alloc(&c->tmp, (size_t)c->n2) != cudaSuccess ||
-        dev_alloc(&c->partial, (size_t)nblk) != cudaSuccess ||
+        dev_alloc(&c->partial, (size_t)nblk * kMultiRhs) != cudaSuccess ||
         dev_alloc(&c->st, 1) != cudaSuccess ||
         dev_alloc(&c->results, (size_t)kMaxShifts + 1) != cudaSuccess)
         return cleanup(QCD_ENOMEM, "qcd_create: device allocation failed");
@@ -479,13 +479,26 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         cur = 1 - cur;
     }
 
-    // finish (a6): true residuals recomputed from x_k, y = sum_k c_k x_k
-    for (int k = 0; k < nshift; ++k) {
-        const double2 *xk = x + h.xoff[k];
-        run_dslash(c, 1 - parity, xk, c->tmp, nullptr, 0.0, false, 0, false);
-        run_dslash(c, parity, c->tmp, c->q, xk, c->mass * c->mass, false, 0, false);
-        c->launches += launch_residual_norm(n2, b, c->q, xk, h.sigma[k], c->partial, c->st,
-                                            c->results + order[k], c->L());
+    // finish (a6): true residuals recomputed from x_k, kMultiRhs shifts per pass over the links;
+    // the p_k are dead by now and serve as the tmp vectors.  y = sum_k c_k x_k.
+    for (int k0 = 0; k0 < nshift; k0 += kMultiRhs) {
+        const int nb = std::min(kMultiRhs, nshift - k0);
+        DslashMultiParams mp{};
+        mp.W = c->W; mp.link_rows = c->link_rows; mp.nrhs = nb;
+        mp.partial = c->partial; mp.counter = &c->st->counter;
+        mp.out_parity = 1 - parity;                      // tmp_j = D_{q,p} x_j
+        mp.in = x; mp.out = c->p;
+        for (int j = 0; j < nb; ++j) { mp.in_off[j] = h.xoff[k0 + j]; mp.out_off[j] = (long long)(k0 + j) * n2; }
+        c->launches += launch_dslash_multi(c->g, mp, c->Ld());
+        mp.out_parity = parity;                          // || b - ((m^2 + sigma_j) x_j - D_{p,q} tmp_j) ||^2
+        mp.in = c->p; mp.out = nullptr; mp.src = x; mp.b = b;
+        for (int j = 0; j < nb; ++j) {
+            mp.in_off[j] = (long long)(k0 + j) * n2;
+            mp.src_off[j] = h.xoff[k0 + j];
+            mp.coeff[j] = c->mass * c->mass + h.sigma[k0 + j];
+            mp.result[j] = c->results + order[k0 + j];
+        }
+        c->launches += launch_dslash_multi(c->g, mp, c->Ld());
     }
     if (d_y)
         c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, c0,

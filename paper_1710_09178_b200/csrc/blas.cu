@@ -120,29 +120,6 @@ cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restr
     }
 }
 
-// *result = || b - (q + sigma x) ||^2   (q == nullptr: *result = ||b||^2)
-__global__ void __launch_bounds__(kBlock)
-residual_norm_kernel(long n2, const double2 *__restrict__ b, const double2 *__restrict__ q,
-                     const double2 *__restrict__ x, double sigma, double *partial, CgState *st,
-                     double *result)
-{
-    pdl_wait();
-    pdl_launch_dependents();
-    double s = 0.0;
-    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
-        double2 d = __ldg(b + i);
-        if (q != nullptr) {
-            const double2 qv = __ldg(q + i), xv = __ldg(x + i);
-            d.x -= fma(sigma, xv.x, qv.x);
-            d.y -= fma(sigma, xv.y, qv.y);
-        }
-        s += d.x * d.x + d.y * d.y;
-    }
-    double total;
-    if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total))
-        if (threadIdx.x == 0) *result = total;
-}
-
 struct CombineArgs {
     long long xoff[kMaxShifts];
     double c[kMaxShifts];
@@ -201,14 +178,6 @@ int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, l
     long units = (n2 + kShiftChunk - 1) / kShiftChunk * kMaxShifts;
     int grid = (int)(units < 148 * 8 ? (units > 0 ? units : 1) : 148 * 8);
     launch_kernel(cg_update_shifts_kernel, grid, kBlock, L.s, L.pdl, n2, r, x, p, pstride, st);
-    return 1;
-}
-
-int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
-                         double *partial, CgState *st, double *result, Launch L)
-{
-    launch_kernel(residual_norm_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, q, x, sigma, partial, st,
-                                                                 result);
     return 1;
 }
 

@@ -143,6 +143,28 @@ int launch_dslash(const Geom &g, const DslashParams &p, Launch L);
 int dslash_grid_blocks(const Geom &g);
 int dslash_chunks(const Geom &g);
 
+// D applied to up to kMultiRhs vectors in one pass over the links (dslash_multi.cu).
+//   b == nullptr:  out_j = D in_j
+//   b != nullptr:  *result[j] = || b - (coeff[j] src_j - D in_j) ||^2, nothing stored
+// vector j lives at base + off[j] (double2 elements).  partial must hold kMultiRhs * grid doubles.
+constexpr int kMultiRhs = 4;
+struct DslashMultiParams {
+    const double2 *W;
+    int link_rows, out_parity, nrhs;
+    const double2 *in;
+    long long in_off[kMultiRhs];
+    double2 *out;
+    long long out_off[kMultiRhs];
+    const double2 *src;
+    long long src_off[kMultiRhs];
+    double coeff[kMultiRhs];
+    const double2 *b;
+    double *partial;
+    unsigned *counter;
+    double *result[kMultiRhs];
+};
+int launch_dslash_multi(const Geom &g, const DslashMultiParams &p, Launch L);
+
 // BLAS-1 (n2 = 3*Vh double2 elements per vector)
 int blas_grid_blocks(long n2);
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
@@ -151,9 +173,6 @@ int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, C
                        Launch L);
 int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
                             CgState *st, Launch L);
-// scratch = || b - (q + sigma x) ||^2   and  scratch = ||b||^2
-int launch_residual_norm(long n2, const double2 *b, const double2 *q, const double2 *x, double sigma,
-                         double *partial, CgState *st, double *result, Launch L);
 // y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
                    int nshift, double c0, const double2 *b, double2 *y, Launch L);

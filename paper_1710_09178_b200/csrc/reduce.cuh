@@ -57,4 +57,34 @@ __device__ __forceinline__ bool grid_sum_last_block(double v, double *partial, u
     return true;
 }
 
+// N sums at once with ONE ticket: partial[blockIdx * N + j].  Returns true in all threads of the block
+// that finishes last, with total[j] = sum over blocks (blockIdx order) of v[j].
+template <int BLOCK, int N>
+__device__ __forceinline__ bool grid_sum_last_block_n(const double (&v)[N], double *partial,
+                                                      unsigned *counter, double (&total)[N])
+{
+    __shared__ bool is_last;
+    double b[N];
+#pragma unroll
+    for (int j = 0; j < N; ++j) b[j] = block_sum<BLOCK>(v[j]);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int j = 0; j < N; ++j) partial[(size_t)blockIdx.x * N + j] = b[j];
+        __threadfence();
+        unsigned ticket = atomicAdd(counter, 1u);
+        is_last = (ticket == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!is_last) return false;
+    __threadfence();
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+        double t = 0.0;
+        for (unsigned i = threadIdx.x; i < gridDim.x; i += BLOCK) t += __ldcg(partial + (size_t)i * N + j);
+        total[j] = block_sum<BLOCK>(t);
+    }
+    if (threadIdx.x == 0) *counter = 0u;
+    return true;
+}
+
 }  // namespace qcd
