@@ -14,9 +14,12 @@ namespace {
 
 constexpr int kBlock = kDslashBlock;
 constexpr int NR = kMultiRhs;
+#ifndef QCD_MULTI_MINB
+#define QCD_MULTI_MINB 4   // 128 registers; measured at 32^3x8 (residual pass): 2 -> 82 us, 3 -> 67, 4 -> 53, 5 (spills) -> 75
+#endif
 
 template <bool RES, int ROWS>
-__global__ void __launch_bounds__(kBlock, 2)
+__global__ void __launch_bounds__(kBlock, QCD_MULTI_MINB)
 dslash_multi_kernel(const Geom g, const DslashMultiParams p)
 {
     constexpr int NW = 3 * ROWS;
