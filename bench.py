@@ -48,7 +48,8 @@ FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
 # summarised in profiles/ (None until a capture for that workload exists).
 # key: (config number, link rows)
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 163.3e6}   # profiles/r01_dslash_full_cfg3.md
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 163.65e6, (3, 2): 110.99e6,   # profiles/r01_dslash_full_cfg3.md
+                             (5, 3): 2.665e9}                       # profiles/r01_dslash_full_cfg5.md
 
 
 def log(*a):
@@ -366,7 +367,9 @@ def main():
         "mdagm": {"us_per_apply": 1e6 * t_b / (K * (PAIRS // 2)), "GBps": mdagm_gbps, "algorithmic_bytes": mdagm_bytes},
         "roofline": {"bound": "hbm", "kernel": "dslash_kernel<false,false> (one D_oe or D_eo apply)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "peak_source": peak_src, "algorithmic_bytes_per_launch": dslash_bytes(V, R), "link_rows": R,
+                     "peak_source": peak_src,
+                     "peak_note": "hbm_gbs is a copy (read+write) rate; this kernel is 96 % reads, so frac "
+                                  "can exceed 1 (read-only probe of the same pattern: DESIGN.md section 5)", "algorithmic_bytes_per_launch": dslash_bytes(V, R), "link_rows": R,
                      "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((cfg.number, R))},
         "gpu_launches": K * (launches_a + launches_b + cg_launches),
     }
