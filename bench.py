@@ -138,24 +138,35 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_sample(cfg, links, b, shifts, res, n_pairs: int, cg_iters: int):
-    """Time the oracle as it stands on the host cores on a bounded sample of the workload."""
+def oracle_sample(cfg, links, b, shifts, res, dslash_seconds: float = 6.0, cg_seconds: float = 12.0):
+    """Time the oracle as it stands on the host cores on a bounded sample of the workload: (D_oe, D_eo)
+    pairs on the full lattice for about `dslash_seconds`, then the multishift CG at the requested tol
+    for as many iterations as fit in about `cg_seconds` (the whole solve if it fits)."""
     import oracle
     lat = oracle.Lattice(cfg.dims, links)
     vo = lat.dslash(1, b)                       # warm-up, also the odd vector
+    n_pairs = 0
     t0 = time.perf_counter()
-    for _ in range(n_pairs):
+    while True:
         vo = lat.dslash(1, b)
         ve = lat.dslash(0, vo)
-    t_d = time.perf_counter() - t0
+        n_pairs += 1
+        t_d = time.perf_counter() - t0
+        if t_d >= dslash_seconds:
+            break
     del ve
     gbps = 2 * n_pairs * dslash_bytes(cfg.volume) / t_d / 1e9
     t0 = time.perf_counter()
-    out = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=cg_iters,
-                            want_x=False)
+    probe = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=3, want_x=False)
+    per_it = (time.perf_counter() - t0) / max(probe["iterations"], 1)
+    iters = max(3, int(cg_seconds / per_it))
+    t0 = time.perf_counter()
+    out = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=iters, want_x=False)
     t_cg = time.perf_counter() - t0
-    return dict(gbps=gbps, dslash_s=t_d / (2 * n_pairs), cg_s_per_iter=t_cg / max(out["iterations"], 1),
-                cg_iters=out["iterations"], cores=oracle.threads(), seconds=t_d + t_cg)
+    return dict(gbps=gbps, dslash_s=t_d / (2 * n_pairs), pairs=n_pairs,
+                cg_s_per_iter=t_cg / max(out["iterations"], 1), cg_iters=out["iterations"],
+                cg_converged=out["status"] == 0, cg_seconds=t_cg,
+                cores=oracle.threads(), seconds=t_d + t_cg)
 
 
 def run_reference(args, cfg, links, b, shifts, res):
@@ -466,13 +477,15 @@ def main():
             ctx.set_option(q.QCD_OPT_LINK_ROWS, 3)
 
         if not args.no_cpu_baseline:
-            pairs = 4 if V <= 262144 else 1
-            smp = oracle_sample(cfg, links, b, shifts, res, n_pairs=pairs, cg_iters=10)
+            smp = oracle_sample(cfg, links, b, shifts, res)
             line["cpu_baseline"] = {
                 "value": smp["gbps"], "unit": UNIT, "cores": smp["cores"], "kind": "oracle",
-                "sample": f"{pairs} x (D_oe, D_eo) on the full {cfg.name} lattice + 10 iterations of the "
-                          f"{cfg.nshift}-shift CG ({smp['seconds']:.1f} s of host time)",
+                "sample": f"{smp['pairs']} x (D_oe, D_eo) on the full {cfg.name} lattice + {smp['cg_iters']} "
+                          f"iterations of the {cfg.nshift}-shift CG"
+                          f"{' (the whole solve)' if smp['cg_converged'] else ''} "
+                          f"({smp['seconds']:.1f} s of host time)",
                 "dslash_us_per_apply": 1e6 * smp["dslash_s"], "cg_s_per_iteration": smp["cg_s_per_iter"],
+                "cg_s_sampled": smp["cg_seconds"], "cg_converged_in_sample": smp["cg_converged"],
                 "host_cpu_count": os.cpu_count()}
         print(json.dumps(line), flush=True)
 
