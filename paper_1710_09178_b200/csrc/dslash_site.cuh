@@ -99,6 +99,11 @@ __device__ __forceinline__ void locate(const Geom &g, int par, Site &s)
         s.hm[2] = (int)h + (z == 0 ? (g.Nz - 1) * g.sz : -g.sz);
         s.hp[3] = (int)h + ((int)t + 1 == g.Nt ? -(g.Nt - 1) * g.st : g.st);
         s.hm[3] = (int)h + (t == 0 ? (g.Nt - 1) * g.st : -g.st);
+#ifdef QCD_DEBUG_BOUNDS   // build with QCD_NVCC_EXTRA=-DQCD_DEBUG_BOUNDS: any neighbour outside [0, Vh) traps
+        for (int mu = 0; mu < 4; ++mu)
+            if ((unsigned)s.hp[mu] >= (unsigned)g.Vh || (unsigned)s.hm[mu] >= (unsigned)g.Vh || h >= (uint32_t)g.Vh)
+                __trap();
+#endif
         if (SIGNS) {
             const int x = 2 * (int)xh + r;
             s.nf[1] = s.nb[1] = x & 1;                   // eta_1 = (-1)^x
