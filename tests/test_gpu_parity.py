@@ -334,6 +334,55 @@ def test_freezing_light_mass_16_shifts(torch, q):
         assert rel_l2(out["x"][k], exact["x"][k]) <= TOL_X
 
 
+def test_maximum_number_of_shifts(torch, q):
+    """QCD_MAX_SHIFTS = 64 shifts in one solve (16 batches of the multi-RHS finish); 65 is refused."""
+    dims, mass = (4, 4, 4, 6), 0.2
+    rig = make_rig(torch, q, dims, "random", mass, 13)
+    b = li.make_source(dims, 13, E)
+    shifts = np.logspace(-3, 1, 64)[::-1].copy()          # descending: the library sorts
+    res = np.linspace(0.5, 1.5, 64)
+    out = rig.solve(E, b, shifts, res, 1e-10)
+    assert out["status"] == 0 and (out["true_res"] <= 1.5e-10).all()
+    for k in (0, 17, 40, 63):
+        xs, _, tr, st = rig.lat.cg(mass, E, shifts[k], b, 1e-14, max_iter=5000)
+        assert st == 0 and rel_l2(out["x"][k], xs) <= TOL_X
+        r = b - (rig.lat.mdagm(mass, E, out["x"][k]) + shifts[k] * out["x"][k])
+        tr = np.linalg.norm(r) / np.linalg.norm(b)
+        assert abs(tr - out["true_res"][k]) <= 1e-3 * tr + 1e-15
+    assert rel_l2(out["y"], np.tensordot(res, out["x"], axes=(0, 0))) <= 1e-14
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.solve(E, b, np.ones(65), np.ones(65), 1e-10)
+
+
+def test_dslash_inside_a_cuda_graph_replay_is_bit_identical(torch, q):
+    """bench.py times graph replays of the Dslash on a side stream: same kernels, same bits."""
+    dims = (12, 6, 10, 4)
+    rig = make_rig(torch, q, dims, "near_identity", 0.07, 5)
+    v = li.make_source(dims, 5, E)
+    d_in, d_o, d_e = rig.to_internal(E, v), rig.ctx.new_vector(), rig.ctx.new_vector()
+    rig.ctx.dslash(O, d_in, d_o)
+    rig.ctx.dslash(E, d_o, d_e)
+    ref_o, ref_e = rig.to_canonical(O, d_o), rig.to_canonical(E, d_e)
+    d_o.zero_(); d_e.zero_()
+    main = torch.cuda.current_stream()
+    side = torch.cuda.Stream()
+    side.wait_stream(main)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        rig.ctx.set_stream(side.cuda_stream)
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(3):
+                rig.ctx.dslash(O, d_in, d_o)
+                rig.ctx.dslash(E, d_o, d_e)
+    rig.ctx.set_stream(main.cuda_stream)
+    main.wait_stream(side)
+    d_o.zero_(); d_e.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(rig.to_canonical(O, d_o), ref_o) and np.array_equal(rig.to_canonical(E, d_e), ref_e)
+    assert rel_l2(ref_o, rig.lat.dslash(O, v)) <= TOL_OP
+
+
 def test_max_iter_and_zero_source(torch, q):
     cfg, links, b, shifts, res = li.make_config_inputs(1)
     rig = Rig(torch, q, cfg.dims, cfg.mass, links)
