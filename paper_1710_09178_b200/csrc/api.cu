@@ -13,6 +13,8 @@
 
 using namespace qcd;
 
+constexpr int kMaxSlabs = 16;  // t-slabs of the pipelined qcd_dslash_host
+
 struct qcd_ctx {
     Geom g{};
     double mass = 0.0;
@@ -38,6 +40,9 @@ struct qcd_ctx {
     // staging for the *_host entry points
     double *stage_links = nullptr;      // canonical gauge field on device
     double *stage_vec = nullptr;        // one canonical parity vector on device
+    double *stage_out = nullptr;        // second one: output side of the pipelined qcd_dslash_host
+    cudaStream_t s_in = nullptr, s_out = nullptr;        // copy-in / copy-out streams of that pipeline
+    cudaEvent_t ev_pipe[2 * kMaxSlabs + 2] = {};         // [0] start, [1..S] slab uploaded, [S+1..2S] slab computed, last: done
     double2 *hv_a = nullptr, *hv_b = nullptr, *hv_y = nullptr;   // internal vectors
     long launches = 0;
     std::string err;
@@ -248,6 +253,7 @@ qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx
     g.Vh = (int)(V / 2);
     g.sy = g.Nxh; g.sz = g.Nxh * g.Ny; g.st = g.Nxh * g.Ny * g.Nz;
     g.dxh.init(g.Nxh); g.dy.init(g.Ny); g.dz.init(g.Nz);
+    g.t0 = 0; g.nt_run = g.Nt;
     g.chunks = dslash_chunks(g);
     g.tgroup = auto_tgroup(g);
     c->n2 = 3L * g.Vh;
@@ -281,6 +287,10 @@ qcd_status qcd_destroy(qcd_ctx *c)
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaFree(c->W); cudaFree(c->tmp); cudaFree(c->q); cudaFree(c->r); cudaFree(c->p);
     cudaFree(c->xws); cudaFree(c->partial); cudaFree(c->st); cudaFree(c->results);
+    if (c->s_in) cudaStreamDestroy(c->s_in);
+    if (c->s_out) cudaStreamDestroy(c->s_out);
+    for (auto &e : c->ev_pipe) if (e) cudaEventDestroy(e);
+    cudaFree(c->stage_out);
     cudaFree(c->stage_links); cudaFree(c->stage_vec); cudaFree(c->hv_a); cudaFree(c->hv_b);
     cudaFree(c->hv_y);
     if (c->h_state) cudaFreeHost(c->h_state);
@@ -560,13 +570,66 @@ qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, doubl
     if (!c) return QCD_EINVAL;
     if (bad_parity(out_parity) || !h_in || !h_out)
         return fail(c, QCD_EINVAL, "qcd_dslash_host: bad argument");
+    if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_dslash_host: no gauge field loaded");
     qcd_status s = ensure_host_staging(c);
     if (s != QCD_OK) return s;
-    QCD_CUDA(c, cudaMemcpyAsync(c->stage_vec, h_in, c->vec_bytes, cudaMemcpyHostToDevice, c->stream));
-    if ((s = qcd_pack(c, 1 - out_parity, c->stage_vec, (double *)c->hv_a)) != QCD_OK) return s;
-    if ((s = qcd_dslash(c, out_parity, (double *)c->hv_a, (double *)c->hv_b)) != QCD_OK) return s;
-    if ((s = qcd_unpack(c, out_parity, (double *)c->hv_b, c->stage_vec)) != QCD_OK) return s;
-    QCD_CUDA(c, cudaMemcpyAsync(h_out, c->stage_vec, c->vec_bytes, cudaMemcpyDeviceToHost, c->stream));
+    // Pipeline over t-slabs: a slab of the canonical vector is one contiguous range of sites, and
+    // the stencil of slab i needs slabs i-1, i, i+1 only.  Upload + pack on one stream, Dslash +
+    // unpack of a slab on the context's stream as soon as its neighbours have arrived, download on a
+    // third stream: the PCIe link runs in both directions at once and the kernels hide behind it.
+    // Slabs: the largest divisor of Nt (at most kMaxSlabs) that keeps a slab at 1.5 MB or more: below
+    // that the ~6 API calls per slab cost more host time than the transfer they overlap.  The last
+    // three slabs can only be computed after the last upload, so more slabs mean a shorter tail.
+    int S = 1;
+    for (int cand = kMaxSlabs; cand >= 3; --cand)
+        if (c->g.Nt % cand == 0 && c->vec_bytes / cand >= (3u << 19)) { S = cand; break; }
+    if (S < 3) {                                    // too few t-slices, or too small to be worth it
+        QCD_CUDA(c, cudaMemcpyAsync(c->stage_vec, h_in, c->vec_bytes, cudaMemcpyHostToDevice, c->stream));
+        if ((s = qcd_pack(c, 1 - out_parity, c->stage_vec, (double *)c->hv_a)) != QCD_OK) return s;
+        if ((s = qcd_dslash(c, out_parity, (double *)c->hv_a, (double *)c->hv_b)) != QCD_OK) return s;
+        if ((s = qcd_unpack(c, out_parity, (double *)c->hv_b, c->stage_vec)) != QCD_OK) return s;
+        QCD_CUDA(c, cudaMemcpyAsync(h_out, c->stage_vec, c->vec_bytes, cudaMemcpyDeviceToHost, c->stream));
+        QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+        return QCD_OK;
+    }
+    if (!c->stage_out) QCD_CUDA(c, cudaMalloc((void **)&c->stage_out, c->vec_bytes));
+    if (!c->s_in) QCD_CUDA(c, cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+    if (!c->s_out) QCD_CUDA(c, cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+    for (int i = 0; i < 2 * S + 2; ++i)
+        if (!c->ev_pipe[i]) QCD_CUDA(c, cudaEventCreateWithFlags(&c->ev_pipe[i], cudaEventDisableTiming));
+    cudaEvent_t ev_start = c->ev_pipe[0], ev_done = c->ev_pipe[2 * S + 1];
+    cudaEvent_t *ev_up = &c->ev_pipe[1], *ev_cmp = &c->ev_pipe[1 + S];
+    const int nts = c->g.Nt / S;                    // t-slices per slab
+    const int hs = nts * c->g.st;                   // sites per slab
+    const size_t slab_doubles = (size_t)hs * 6, slab_bytes = slab_doubles * sizeof(double);
+    const Launch Lin{c->s_in, c->opt_pdl, nullptr};
+    QCD_CUDA(c, cudaEventRecord(ev_start, c->stream));      // order after earlier work on the user's stream
+    QCD_CUDA(c, cudaStreamWaitEvent(c->s_in, ev_start, 0));
+    QCD_CUDA(c, cudaStreamWaitEvent(c->s_out, ev_start, 0));
+    for (int i = 0; i < S; ++i) {
+        QCD_CUDA(c, cudaMemcpyAsync(c->stage_vec + i * slab_doubles, h_in + i * slab_doubles, slab_bytes,
+                                    cudaMemcpyHostToDevice, c->s_in));
+        c->launches += launch_pack(c->g, c->stage_vec, c->hv_a, Lin, i * hs, (i + 1) * hs);
+        QCD_CUDA(c, cudaEventRecord(ev_up[i], c->s_in));
+    }
+    for (int n = 0; n < S; ++n) {
+        const int i = n < S - 1 ? n + 1 : 0;         // slabs 1 .. S-1, then slab 0 (it needs slab S-1)
+        const int need = i == 0 ? S - 1 : std::min(i + 1, S - 1);   // uploads complete in order
+        QCD_CUDA(c, cudaStreamWaitEvent(c->stream, ev_up[need], 0));
+        Geom g = c->g;
+        g.t0 = i * nts; g.nt_run = nts;
+        DslashParams p{};
+        p.W = c->W; p.link_rows = c->link_rows; p.in = c->hv_a; p.out = c->hv_b; p.out_parity = out_parity;
+        c->launches += launch_dslash(g, p, c->Ld());
+        c->launches += launch_unpack(c->g, c->hv_b, c->stage_out, c->L(), i * hs, (i + 1) * hs);
+        QCD_CUDA(c, cudaEventRecord(ev_cmp[i], c->stream));
+        QCD_CUDA(c, cudaStreamWaitEvent(c->s_out, ev_cmp[i], 0));
+        QCD_CUDA(c, cudaMemcpyAsync(h_out + i * slab_doubles, c->stage_out + i * slab_doubles, slab_bytes,
+                                    cudaMemcpyDeviceToHost, c->s_out));
+    }
+    QCD_CUDA(c, cudaEventRecord(ev_done, c->s_out));
+    QCD_CUDA(c, cudaStreamWaitEvent(c->stream, ev_done, 0));
+    if ((s = check_launch(c, "qcd_dslash_host")) != QCD_OK) return s;
     QCD_CUDA(c, cudaStreamSynchronize(c->stream));
     return QCD_OK;
 }

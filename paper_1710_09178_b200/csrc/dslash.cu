@@ -110,7 +110,7 @@ dslash_kernel(const Geom g, const DslashParams p)
 }  // namespace
 
 int dslash_chunks(const Geom &g) { return (g.st + kBlock - 1) / kBlock; }
-int dslash_grid_blocks(const Geom &g) { return dslash_chunks(g) * g.Nt; }
+int dslash_grid_blocks(const Geom &g) { return dslash_chunks(g) * g.nt_run; }
 
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
 {

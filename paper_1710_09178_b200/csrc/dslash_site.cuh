@@ -63,7 +63,8 @@ struct Site {
 
 // CTA order.  A chunk is kDslashBlock consecutive sites of one t-slice.  The chunks of a slice are
 // cut into groups of g.tgroup; CTAs walk group by group, and inside a group t runs slowest:
-//     blockIdx = (group * Nt + t) * tgroup + chunk_in_group        (last group may be shorter)
+//     blockIdx = (group * nt_run + t - t0) * tgroup + chunk_in_group   (last group may be shorter;
+//     a launch covers the t-slices t0 <= t < t0 + nt_run, normally all Nt of them)
 // so the CTAs that read the same input sites as +-t neighbours are tgroup CTAs apart instead of a
 // whole t-slice of CTAs (1024 CTAs = 163 MB of link traffic at 64^3x16, more than L2 holds: ncu
 // showed 2.7-2.8 GB of DRAM reads per apply against 2.52 GB algorithmic), while each group still
@@ -72,12 +73,13 @@ struct Site {
 template <bool SIGNS>
 __device__ __forceinline__ void locate(const Geom &g, int par, Site &s)
 {
-    const uint32_t per_group = (uint32_t)g.tgroup * (uint32_t)g.Nt;
+    const uint32_t per_group = (uint32_t)g.tgroup * (uint32_t)g.nt_run;
     const uint32_t grp = blockIdx.x / per_group, rem = blockIdx.x - grp * per_group;
     const uint32_t first = grp * (uint32_t)g.tgroup;
     const uint32_t width = min((uint32_t)g.tgroup, (uint32_t)g.chunks - first);   // chunks in this group
-    const uint32_t t = rem / width;
-    const uint32_t chunk = first + (rem - t * width);
+    const uint32_t tq = rem / width;
+    const uint32_t t = (uint32_t)g.t0 + tq;
+    const uint32_t chunk = first + (rem - tq * width);
     const uint32_t sl = chunk * kDslashBlock + threadIdx.x;    // index inside the t-slice
     s.valid = sl < (uint32_t)g.st;
     const uint32_t h = t * (uint32_t)g.st + sl;

@@ -40,6 +40,7 @@ struct Geom {
     int Vh;          // sites of one parity
     int sy, sz, st;  // half-index strides of +y, +z, +t
     FastDiv dxh, dy, dz;
+    int t0, nt_run;  // t-slices t0 <= t < t0 + nt_run are computed by a Dslash launch (default: all)
     int chunks;      // Dslash CTAs per t-slice
     int tgroup;      // chunks per group of the Dslash CTA order (dslash.cu), 1 <= tgroup <= chunks
 };
@@ -120,8 +121,9 @@ struct Launch {
 };
 
 int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, Launch L);
-int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L);
-int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L);
+// sites h0 <= h < h1 only (h1 < 0: all)
+int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L, int h0 = 0, int h1 = -1);
+int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L, int h0 = 0, int h1 = -1);
 
 struct DslashParams {
     const double2 *W;

@@ -50,25 +50,25 @@ ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__
     }
 }
 
-// canonical parity vector [j][3] (j == h) -> planes [3][Vh]
+// canonical parity vector [j][3] (j == h) -> planes [3][Vh], sites h0 <= h < h1
 __global__ void __launch_bounds__(kBlock)
-pack_kernel(int Vh, const double2 *__restrict__ canon, double2 *__restrict__ v)
+pack_kernel(int Vh, int h0, int h1, const double2 *__restrict__ canon, double2 *__restrict__ v)
 {
     pdl_wait();
     pdl_launch_dependents();
-    int h = blockIdx.x * kBlock + threadIdx.x;
-    if (h >= Vh) return;
+    int h = h0 + blockIdx.x * kBlock + threadIdx.x;
+    if (h >= h1) return;
 #pragma unroll
     for (int c = 0; c < 3; ++c) v[(long)c * Vh + h] = canon[3L * h + c];
 }
 
 __global__ void __launch_bounds__(kBlock)
-unpack_kernel(int Vh, const double2 *__restrict__ v, double2 *__restrict__ canon)
+unpack_kernel(int Vh, int h0, int h1, const double2 *__restrict__ v, double2 *__restrict__ canon)
 {
     pdl_wait();
     pdl_launch_dependents();
-    int h = blockIdx.x * kBlock + threadIdx.x;
-    if (h >= Vh) return;
+    int h = h0 + blockIdx.x * kBlock + threadIdx.x;
+    if (h >= h1) return;
 #pragma unroll
     for (int c = 0; c < 3; ++c) canon[3L * h + c] = v[(long)c * Vh + h];
 }
@@ -85,17 +85,19 @@ int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, in
     return 1;
 }
 
-int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L)
+int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L, int h0, int h1)
 {
-    int blocks = (g.Vh + kBlock - 1) / kBlock;
-    launch_kernel(pack_kernel, blocks, kBlock, L.s, L.pdl, g.Vh, (const double2 *)canon, internal);
+    if (h1 < 0) h1 = g.Vh;
+    int blocks = (h1 - h0 + kBlock - 1) / kBlock;
+    launch_kernel(pack_kernel, blocks, kBlock, L.s, L.pdl, g.Vh, h0, h1, (const double2 *)canon, internal);
     return 1;
 }
 
-int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L)
+int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L, int h0, int h1)
 {
-    int blocks = (g.Vh + kBlock - 1) / kBlock;
-    launch_kernel(unpack_kernel, blocks, kBlock, L.s, L.pdl, g.Vh, internal, (double2 *)canon);
+    if (h1 < 0) h1 = g.Vh;
+    int blocks = (h1 - h0 + kBlock - 1) / kBlock;
+    launch_kernel(unpack_kernel, blocks, kBlock, L.s, L.pdl, g.Vh, h0, h1, internal, (double2 *)canon);
     return 1;
 }
 

@@ -476,6 +476,28 @@ def test_inv_sqrt_argument_errors(torch, q):
         rig.ctx.inv_sqrt(E, v, 4, 0.01, 5.0, 1e-10, 100, v)
 
 
+def test_pipelined_host_dslash(torch, q):
+    """qcd_dslash_host on vectors of 4.5 MB or more runs as a t-slab pipeline (upload / compute /
+    download on three streams; 3 slabs of 4 t-slices here): same bits as the device entry point, and
+    the oracle's operator."""
+    dims = (32, 32, 16, 12)
+    links = li.make_links(dims, "random", 17)
+    for rows in (3, 2):
+        rig = Rig(torch, q, dims, 0.05, links, link_rows=rows)
+        for par in (O, E):
+            v = li.make_source(dims, 3 + par, 1 - par)
+            hin = torch.from_numpy(v).pin_memory().numpy()
+            hout = torch.empty(v.shape, dtype=torch.float64).pin_memory().numpy()
+            for _ in range(2):                      # second call reuses streams and events
+                hout[:] = 0.0
+                rig.ctx.dslash_host(par, hin, hout)
+                assert np.array_equal(hout, rig.dslash(par, v))
+            assert rel_l2(hout, rig.lat.dslash(par, v)) <= TOL_OP
+        out = np.empty_like(v)                      # pageable host memory works too
+        rig.ctx.dslash_host(par, v, out)
+        assert np.array_equal(out, hout)
+
+
 # ------------------------------------------------------------------ full-size configs 3, 4, 5
 
 @pytest.mark.slow
