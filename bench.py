@@ -222,6 +222,7 @@ def main():
     ap.add_argument("--no-solve", action="store_true", help="skip section C (profiling aid)")
     ap.add_argument("--no-pdl", action="store_true", help="QCD_OPT_PDL=0 (A/B aid)")
     ap.add_argument("--no-cg-graph", action="store_true", help="QCD_OPT_CG_GRAPH=0 (A/B aid)")
+    ap.add_argument("--cg-graph", type=int, default=-1, help="QCD_OPT_CG_GRAPH value (-1 = library default)")
     ap.add_argument("--cg-batch", type=int, default=0, help="QCD_OPT_CG_BATCH (0 = library default)")
     ap.add_argument("--link-rows", type=int, default=3, choices=[2, 3],
                     help="QCD_OPT_LINK_ROWS for the whole run (default 3, the paper's uncompressed "
@@ -262,6 +263,8 @@ def main():
         ctx.set_option(q.QCD_OPT_PDL, 0)
     if args.no_cg_graph:
         ctx.set_option(q.QCD_OPT_CG_GRAPH, 0)
+    if args.cg_graph >= 0:
+        ctx.set_option(q.QCD_OPT_CG_GRAPH, args.cg_graph)
     if args.cg_batch:
         ctx.set_option(q.QCD_OPT_CG_BATCH, args.cg_batch)
     ctx.set_option(q.QCD_OPT_LINK_ROWS, args.link_rows)

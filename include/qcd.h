@@ -73,8 +73,13 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 /* Execution options.  PDL, CG_GRAPH and CG_BATCH leave every result bit-identical.
  *   QCD_OPT_PDL       (default 1) launch every kernel with programmatic dependent launch, so that its
  *                     index arithmetic overlaps the tail of its predecessor in the stream or graph.
- *   QCD_OPT_CG_GRAPH  (default 1) qcd_multishift_cg replays one captured CUDA graph per batch of
- *                     iterations instead of launching 4 kernels per iteration from the host.
+ *   QCD_OPT_CG_GRAPH  (default 1) how qcd_multishift_cg enqueues its iterations.  0: four kernel launches
+ *                     per iteration from the host.  1: one captured CUDA graph per batch of iterations.
+ *                     2: ONE graph for the whole solve, a WHILE conditional node whose body is one
+ *                     iteration and whose condition the device-side stop test sets: no early-exit
+ *                     launches after convergence, no host polling.  Measured on B200 it is no faster
+ *                     than 1 (7.93 vs 7.84 ms at 32^3x8, 5.69 vs 5.31 ms at 4^4): the loop node costs
+ *                     about 1 us per iteration and breaks the PDL chain between iterations.
  *   QCD_OPT_CG_BATCH  (default 8) iterations per batch; the host reads the device's convergence flag
  *                     once per batch, one batch late, so up to 2 batches of early-exit kernels follow
  *                     convergence.  1 <= value <= 1024.

@@ -48,7 +48,8 @@ struct qcd_ctx {
     std::string err;
     // options (qcd_set_option)
     bool opt_pdl = true;                // programmatic dependent launch on every kernel
-    bool opt_cg_graph = true;           // replay one captured graph per batch of CG iterations
+    int opt_cg_graph = 1;               // 0: plain launches; 1: one captured graph per batch; 2: device-side WHILE loop
+    unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
     int opt_cg_batch = 8;               // iterations enqueued per batch / per graph
     // cached graph of one batch of CG iterations (valid for exactly the key below)
     cudaGraphExec_t cg_exec = nullptr;
@@ -177,11 +178,12 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x)
     // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
     run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
     run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
-    c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->partial, c->st, c->L());
+    c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->partial, c->st, c->loop_handle, c->L());
     c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
 }
 
-// Capture `batch` iterations into a graph (once per distinct set of buffers, parity and mass).
+// Capture `batch` iterations into a graph (once per distinct set of buffers, parity and mass);
+// batch == 0: the device-side loop graph.
 qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
 {
     qcd_ctx::CgKey key;
@@ -194,11 +196,42 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
     cudaStream_t user = c->stream;
     const long launches0 = c->launches;
     c->stream = c->cap_stream;
-    cudaError_t e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
-    if (e == cudaSuccess) {
-        for (int i = 0; i < batch; ++i) enqueue_cg_iteration(c, parity, x);
+    cudaError_t e;
+    if (batch > 0) {
+        e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+            for (int i = 0; i < batch; ++i) enqueue_cg_iteration(c, parity, x);
+            cudaGraph_t graph = nullptr;
+            e = cudaStreamEndCapture(c->cap_stream, &graph);
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
+            if (graph) cudaGraphDestroy(graph);
+        }
+    } else {
+        // batch == 0: ONE graph for the whole solve.  A WHILE conditional node whose body is one CG
+        // iteration; the r-update's last block sets the condition from the device-side stop test, so
+        // the loop ends right after the converging iteration: no dead launches, no host polling.
         cudaGraph_t graph = nullptr;
-        e = cudaStreamEndCapture(c->cap_stream, &graph);
+        cudaGraphConditionalHandle handle = 0;
+        e = cudaGraphCreate(&graph, 0);
+        if (e == cudaSuccess) e = cudaGraphConditionalHandleCreate(&handle, graph, 1, cudaGraphCondAssignDefault);
+        cudaGraphNodeParams np{};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = handle;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t node = nullptr;
+        if (e == cudaSuccess) e = cudaGraphAddNode(&node, graph, nullptr, 0, &np);
+        if (e == cudaSuccess) {
+            cudaGraph_t body = np.conditional.phGraph_out[0];
+            e = cudaStreamBeginCaptureToGraph(c->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+            if (e == cudaSuccess) {
+                c->loop_handle = (unsigned long long)handle;
+                enqueue_cg_iteration(c, parity, x);
+                c->loop_handle = 0;
+                cudaGraph_t same = nullptr;
+                e = cudaStreamEndCapture(c->cap_stream, &same);
+            }
+        }
         if (e == cudaSuccess) e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
         if (graph) cudaGraphDestroy(graph);
     }
@@ -321,7 +354,10 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
     if (!c) return QCD_EINVAL;
     switch (option) {
     case QCD_OPT_PDL: c->opt_pdl = value != 0; return QCD_OK;
-    case QCD_OPT_CG_GRAPH: c->opt_cg_graph = value != 0; return QCD_OK;
+    case QCD_OPT_CG_GRAPH:
+        if (value < 0 || value > 2) return fail(c, QCD_EINVAL, "qcd_set_option: CG graph mode must be 0, 1 or 2");
+        c->opt_cg_graph = (int)value;
+        return QCD_OK;
     case QCD_OPT_CG_BATCH:
         if (value < 1 || value > 1024) return fail(c, QCD_EINVAL, "qcd_set_option: batch must be in [1, 1024]");
         c->opt_cg_batch = (int)value;
@@ -464,7 +500,11 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
 
     // iteration loop: enqueue only (one graph replay, or 4 launches per iteration, per batch)
     const int batch = std::max(1, std::min(c->opt_cg_batch, max_iter));
-    const bool use_graph = c->opt_cg_graph;
+    const bool use_graph = c->opt_cg_graph == 1;
+    if (c->opt_cg_graph == 2) {
+        if ((s = ensure_cg_graph(c, parity, x, 0)) != QCD_OK) return s;
+        QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));     // launch count added below, once iter is known
+    } else {
     if (use_graph && (s = ensure_cg_graph(c, parity, x, batch)) != QCD_OK) return s;
     int enq = 0, cur = 0;
     bool pending = false, finished = false;
@@ -487,6 +527,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         QCD_CUDA(c, cudaEventRecord(c->ev[cur], st));
         pending = true;
         cur = 1 - cur;
+    }
     }
 
     // finish (a6): true residuals recomputed from x_k, kMultiRhs shifts per pass over the links;
@@ -520,6 +561,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     QCD_CUDA(c, cudaStreamSynchronize(st));
 
     *iterations = h.iter;
+    if (c->opt_cg_graph == 2) c->launches += 4L * std::max(h.iter, 1);   // the loop body ran once per iteration
     const double rho_b = h.rho_b;
     for (int k = 0; k < nshift; ++k)
         true_res[k] = rho_b > 0.0 ? std::sqrt(c->h_results[k] / rho_b) : 0.0;

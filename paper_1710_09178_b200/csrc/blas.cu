@@ -41,12 +41,15 @@ cg_init_kernel(long n2, const double2 *__restrict__ b, double2 *__restrict__ r,
 // r -= alpha q ; rho' = <r,r> ; last block: beta, beta_k, zeta rotation, freezing, stop test
 __global__ void __launch_bounds__(kBlock)
 cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q, double *partial,
-                   CgState *st)
+                   CgState *st, cudaGraphConditionalHandle loop)
 {
     pdl_wait();
     pdl_launch_dependents();
     if (st->done) {                       // dead iteration after convergence
-        if (blockIdx.x == 0 && threadIdx.x == 0) st->done_prev = 1;
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            st->done_prev = 1;
+            if (loop) cudaGraphSetConditional(loop, 0);
+        }
         return;
     }
     const double alpha = st->alpha;
@@ -60,7 +63,12 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
         s += rv.x * rv.x + rv.y * rv.y;
     }
     double total;
-    if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total)) cg_step_beta(st, total);
+    if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total)) {
+        cg_step_beta(st, total);
+        // device-side loop (QCD_OPT_CG_GRAPH = 2): this iteration's shift update still runs (it is part
+        // of the loop body); the WHILE node then stops when the stop test above has set `done`
+        if (loop && threadIdx.x == 0) cudaGraphSetConditional(loop, st->done ? 0u : 1u);
+    }
 }
 
 // for every shift k updated this iteration:  x_k += alpha_k p_k ;  p_k = zeta_k^new r + beta_k p_k
@@ -165,9 +173,10 @@ int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstri
 }
 
 int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
-                       Launch L)
+                       unsigned long long loop_handle, Launch L)
 {
-    launch_kernel(cg_update_r_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st);
+    launch_kernel(cg_update_r_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st,
+                  (cudaGraphConditionalHandle)loop_handle);
     return 1;
 }
 

@@ -171,8 +171,9 @@ int launch_dslash_multi(const Geom &g, const DslashMultiParams &p, Launch L);
 int blas_grid_blocks(long n2);
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
                    double *partial, CgState *st, Launch L);
+// loop_handle != 0: the kernel is a node of a WHILE conditional graph and sets its condition
 int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
-                       Launch L);
+                       unsigned long long loop_handle, Launch L);
 int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
                             CgState *st, Launch L);
 // y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)

@@ -251,7 +251,7 @@ def test_execution_options_do_not_change_a_single_bit(torch, q):
     rig = Rig(torch, q, cfg.dims, cfg.mass, links)
     ref = rig.solve(E, b, shifts, res, cfg.tol)
     ref_d = rig.dslash(O, b)
-    for pdl, graph, batch in [(0, 0, 16), (1, 0, 3), (0, 1, 1), (1, 1, 5), (1, 1, 64)]:
+    for pdl, graph, batch in [(0, 0, 16), (1, 0, 3), (0, 1, 1), (1, 1, 5), (1, 1, 64), (1, 2, 8), (0, 2, 8)]:
         rig.ctx.set_option(q.QCD_OPT_PDL, pdl)
         rig.ctx.set_option(q.QCD_OPT_CG_GRAPH, graph)
         rig.ctx.set_option(q.QCD_OPT_CG_BATCH, batch)
@@ -260,6 +260,15 @@ def test_execution_options_do_not_change_a_single_bit(torch, q):
         assert np.array_equal(out["x"], ref["x"]) and np.array_equal(out["y"], ref["y"])
         assert np.array_equal(out["true_res"], ref["true_res"])
         assert np.array_equal(rig.dslash(O, b), ref_d)
+    # device-side loop: max_iter and the zero source end the WHILE node too
+    cut = rig.solve(E, b, shifts, res, cfg.tol, max_iter=7)
+    assert cut["status"] == 4 and cut["iterations"] == 7
+    zero = rig.solve(E, np.zeros_like(b), shifts, res, cfg.tol)
+    assert zero["status"] == 0 and zero["iterations"] == 0 and not zero["x"].any()
+    again = rig.solve(E, b, shifts, res, cfg.tol)
+    assert np.array_equal(again["x"], ref["x"])
+    with pytest.raises(q.QcdError):
+        rig.ctx.set_option(q.QCD_OPT_CG_GRAPH, 3)
     with pytest.raises(q.QcdError):
         rig.ctx.set_option(q.QCD_OPT_CG_BATCH, 0)
     with pytest.raises(q.QcdError):
