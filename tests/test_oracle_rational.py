@@ -112,3 +112,59 @@ def test_eq8_on_a_dense_operator():
     # and the same through the eigen-decomposition (eq. 8 as a scalar identity)
     r = np.asarray(R.eval_eq8(z["c0"], z["c"], z["d"], lam), dtype=float)
     assert np.abs(r * np.sqrt(lam) - 1).max() <= 1.0001 * z["delta"]
+
+
+# ------------------------------------------------------------------ any exponent (x^(1/4))
+
+from fractions import Fraction  # noqa: E402
+
+
+@pytest.mark.parametrize("alpha,n,xmin,xmax", [(Fraction(1, 4), 6, 1e-3, 7.0), (Fraction(-1, 4), 5, 1e-2, 9.0),
+                                               (Fraction(1, 4), 10, 2.5e-5, 8.5)])
+def test_minimax_pow_equioscillates(alpha, n, xmin, xmax):
+    """Chebyshev's criterion again: 2n+2 alternating extrema of equal size of r(x)/x^alpha - 1."""
+    z = R.minimax_pow(alpha, n, xmin, xmax)
+    x = xmin * (xmax / xmin) ** (np.arange(6001) / 6000.0)
+    err = R.relative_error_curve_pow(float(alpha), z["c0"], z["c"], z["d"], x)
+    ext = _extrema(err)
+    assert len(ext) == 2 * n + 2 and ext[0] == 0 and ext[-1] == len(x) - 1
+    signs = np.sign(err[ext])
+    assert (signs[1:] * signs[:-1] < 0).all()
+    assert np.abs(np.abs(err[ext]) / z["delta"] - 1).max() < 2e-4
+    assert abs(np.abs(err).max() / z["delta"] - 1) < 1e-6
+    assert (z["d"] > 0).all() and (np.diff(z["d"]) > 0).all()
+    # x^alpha with alpha > 0 grows: negative residues; alpha < 0: positive (Stieltjes function)
+    assert (z["c"] * np.sign(float(alpha)) < 0).all() and z["c0"] > 0
+
+
+def test_minimax_pow_reproduces_the_closed_form_at_minus_one_half():
+    """The general routine run at alpha = -1/2 must land on Zolotarev's solution (pinned above)."""
+    z = R.minimax_pow(Fraction(-1, 2), 7, 3e-4, 8.5)
+    zz = R.zolotarev_inv_sqrt(7, 3e-4, 8.5)
+    assert abs(z["c0"] / zz["c0"] - 1) < 1e-13 and abs(z["delta"] / zz["delta"] - 1) < 1e-9
+    assert np.abs(z["c"] / zz["c"] - 1).max() < 1e-13 and np.abs(z["d"] / zz["d"] - 1).max() < 1e-13
+
+
+def test_minimax_pow_fourth_power_and_inverse():
+    z = R.minimax_pow(Fraction(1, 4), 9, 1e-4, 8.5)
+    x = np.logspace(-4, np.log10(8.5), 499)
+    r = R.eval_eq8(z["c0"], z["c"], z["d"], x)
+    assert np.abs(r ** 4 / x - 1).max() <= 4.1 * z["delta"]
+    zi = R.minimax_pow(Fraction(-1, 4), 9, 1e-4, 8.5)        # x^(1/4) x^(-1/4) = 1
+    ri = R.eval_eq8(zi["c0"], zi["c"], zi["d"], x)
+    assert np.abs(r * ri - 1).max() <= 1.01 * (z["delta"] + zi["delta"])
+    assert z["delta"] < 1e-5 and zi["delta"] < 1e-5
+
+
+def test_fourth_root_on_a_dense_operator():
+    """(M^dag M)^(1/4) phi through eigh against eq. 8 with the oracle's multishift solves."""
+    cfg, links, b, _, _ = li.make_config_inputs(1)
+    lat = oracle.Lattice(cfg.dims, links)
+    a = dense_from_operator(lambda v: lat.mdagm(cfg.mass, 0, v), lat.volume // 2)
+    lam, qmat = np.linalg.eigh(a)
+    z = R.minimax_pow(Fraction(1, 4), 10, 0.9 * lam.min(), 1.1 * lam.max())
+    phi = cplx(b).reshape(-1)
+    exact = qmat @ ((qmat.conj().T @ phi) * lam ** 0.25)
+    sol = lat.solve_exact(cfg.mass, 0, b, z["d"], z["c"], 1e-12)
+    got = z["c0"] * phi + cplx(sol["y"]).reshape(-1)
+    assert np.linalg.norm(got - exact) / np.linalg.norm(exact) <= 1.05 * z["delta"] + 1e-12
