@@ -446,6 +446,21 @@ def main():
                                 "what": "qcd_inv_sqrt: Zolotarev coefficients + one multishift CG + "
                                         "fused c0*phi + sum c_k x_k"}
 
+            # ... and the heat-bath power (M^dag M)^(1/4) (Remez coefficients, cached)
+            ts = []
+            for _ in range(3):
+                torch.cuda.synchronize()
+                w0 = time.perf_counter()
+                st, it, tr, delta = ctx.apply_pow(cfg.parity, d_b, 1, 4, cfg.nshift, xmin, xmax, cfg.tol,
+                                                  100000, d_y)
+                ts.append(time.perf_counter() - w0)
+                assert st == 0 and tr.max() <= 1.5 * cfg.tol, (st, tr)
+            line["fourth_root"] = {"n": cfg.nshift, "delta": delta, "iterations": it,
+                                   "s_per_apply": statistics.median(ts[1:]),
+                                   "first_call_s": ts[0],
+                                   "what": "qcd_apply_pow(1/4): Remez coefficients in binary128 on the "
+                                           "first call, then one multishift CG + fused combine"}
+
         if R == 3 and not args.no_two_row:
             # the same sections A and C with two-row link storage
             ctx.set_option(q.QCD_OPT_LINK_ROWS, 2)

@@ -168,6 +168,24 @@ QCD_API qcd_status qcd_inv_sqrt(qcd_ctx *ctx, int parity, const double *d_phi, i
                                 double xmax, double tol, int max_iter, double *d_out,
                                 int *iterations, double *true_res, double *delta);
 
+/* The general exponent of eq. 8, (M^dag M)^(1/b): alpha = num/den with
+ * 0 < |alpha| < 1, in particular the heat-bath power alpha = 1/4 (b = 4, appendix :288-304).
+ *
+ * qcd_pow_coeffs: HOST ONLY.  Minimax (relative error, type (n, n)) approximation
+ *   x^alpha ~= c0 + sum_{k<n} coef[k] / (x + shift[k])  on [xmin, xmax]; shift ascending and > 0; coef < 0
+ * for alpha > 0, > 0 for alpha < 0.  alpha = -1/2 is the closed form of qcd_inv_sqrt_coeffs; any other
+ * exponent runs a Remez exchange iteration in binary128 arithmetic started from that closed form
+ * (about 0.1-1 s).  delta (may be NULL): max |r(x)/x^alpha - 1|.  QCD_EINVAL for bad arguments,
+ * QCD_ENOTCONV if the iteration does not converge (n too large for the interval: delta would be
+ * below ~1e-15).
+ *
+ * qcd_apply_pow: d_out = c0 d_phi + sum_k coef[k] (M^dag M + shift[k])^(-1) d_phi, as qcd_inv_sqrt. */
+QCD_API qcd_status qcd_pow_coeffs(int num, int den, int n, double xmin, double xmax, double *c0,
+                                  double *coef, double *shift, double *delta);
+QCD_API qcd_status qcd_apply_pow(qcd_ctx *ctx, int parity, const double *d_phi, int num, int den, int n,
+                                 double xmin, double xmax, double tol, int max_iter, double *d_out,
+                                 int *iterations, double *true_res, double *delta);
+
 /* Host-buffer forms (canonical layout on the host; H2D copy, pack, compute, unpack, D2H copy and a
  * stream synchronise all happen inside the call).  h_x: nshift canonical parity vectors or NULL;
  * h_y: one canonical parity vector or NULL. */

@@ -43,6 +43,8 @@ _SIGNATURES = {
                                 ctypes.POINTER(_ci), _vp]),
     "qcd_inv_sqrt_coeffs": (_ci, [_ci, _cd, _cd, _vp, _vp, _vp, _vp]),
     "qcd_inv_sqrt": (_ci, [_vp, _ci, _vp, _ci, _cd, _cd, _cd, _ci, _vp, ctypes.POINTER(_ci), _vp, _vp]),
+    "qcd_pow_coeffs": (_ci, [_ci, _ci, _ci, _cd, _cd, _vp, _vp, _vp, _vp]),
+    "qcd_apply_pow": (_ci, [_vp, _ci, _vp, _ci, _ci, _ci, _cd, _cd, _cd, _ci, _vp, ctypes.POINTER(_ci), _vp, _vp]),
     "qcd_dslash_host": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_mdagm_host": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_multishift_cg_host": (_ci, [_vp, _ci, _vp, _ci, _vp, _vp, _cd, _ci, _vp, _vp,
@@ -124,6 +126,18 @@ def inv_sqrt_coeffs(n: int, xmin: float, xmax: float):
                                  _host_ptr(d), _host_ptr(delta))
     if st != QCD_OK:
         raise QcdError(st, "qcd_inv_sqrt_coeffs", lib.qcd_last_error(None).decode())
+    return float(c0[0]), c, d, float(delta[0])
+
+
+def pow_coeffs(num: int, den: int, n: int, xmin: float, xmax: float):
+    """qcd_pow_coeffs (host only): x^(num/den) ~= c0 + sum c[k]/(x + d[k]); returns (c0, c, d, delta)."""
+    lib = load_library()
+    c0, delta = np.zeros(1), np.zeros(1)
+    c, d = np.zeros(max(int(n), 1)), np.zeros(max(int(n), 1))
+    st = lib.qcd_pow_coeffs(int(num), int(den), int(n), float(xmin), float(xmax), _host_ptr(c0),
+                            _host_ptr(c), _host_ptr(d), _host_ptr(delta))
+    if st != QCD_OK:
+        raise QcdError(st, "qcd_pow_coeffs", lib.qcd_last_error(None).decode())
     return float(c0[0]), c, d, float(delta[0])
 
 
@@ -219,6 +233,19 @@ class Context:
                                     float(tol), int(max_iter), _dev_ptr(d_out), ctypes.byref(it),
                                     _host_ptr(true_res), _host_ptr(delta))
         self._check(st, "qcd_inv_sqrt", allow=(QCD_ENOTCONV,))
+        return st, it.value, true_res, float(delta[0])
+
+    def apply_pow(self, parity: int, d_phi, num: int, den: int, n: int, xmin: float, xmax: float,
+                  tol: float, max_iter: int, d_out):
+        """Returns (status, iterations, true_res[n], delta)."""
+        true_res = np.full(int(n), np.nan)
+        delta = np.zeros(1)
+        it = _ci(0)
+        st = self._lib.qcd_apply_pow(self._h, parity, _dev_ptr(d_phi), int(num), int(den), int(n),
+                                     float(xmin), float(xmax), float(tol), int(max_iter),
+                                     _dev_ptr(d_out), ctypes.byref(it), _host_ptr(true_res),
+                                     _host_ptr(delta))
+        self._check(st, "qcd_apply_pow", allow=(QCD_ENOTCONV,))
         return st, it.value, true_res, float(delta[0])
 
     # -- host entry points (canonical numpy arrays; copies happen inside the C call) --

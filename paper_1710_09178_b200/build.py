@@ -39,7 +39,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB + f".{os.getpid()}.tmp"
     extra = os.environ.get("QCD_NVCC_EXTRA", "").split()       # e.g. -DQCD_DSLASH2_MINB=6 (tuning aid)
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + sources()
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-o", tmp] + sources() + ["-lquadmath"]
     subprocess.run(cmd, check=True)
     os.replace(tmp, LIB)
     return LIB

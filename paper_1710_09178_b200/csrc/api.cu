@@ -45,6 +45,9 @@ struct qcd_ctx {
     cudaEvent_t ev_pipe[2 * kMaxSlabs + 2] = {};         // [0] start, [1..S] slab uploaded, [S+1..2S] slab computed, last: done
     double2 *hv_a = nullptr, *hv_b = nullptr, *hv_y = nullptr;   // internal vectors
     long launches = 0;
+    // coefficients of qcd_apply_pow, cached per (num, den, n, xmin, xmax): the Remez run takes ~1 s
+    struct PowFit { int num, den, n; double xmin, xmax, c0, delta; std::vector<double> coef, shift; };
+    std::vector<PowFit> pow_cache;
     std::string err;
     // options (qcd_set_option)
     bool opt_pdl = true;                // programmatic dependent launch on every kernel
@@ -592,6 +595,43 @@ qcd_status qcd_inv_sqrt_coeffs(int n, double xmin, double xmax, double *c0, doub
         return fail(nullptr, QCD_EINVAL,
                     "qcd_inv_sqrt_coeffs: need 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax");
     return QCD_OK;
+}
+
+qcd_status qcd_pow_coeffs(int num, int den, int n, double xmin, double xmax, double *c0,
+                          double *coef, double *shift, double *delta)
+{
+    if (!c0 || !coef || !shift) return fail(nullptr, QCD_EINVAL, "qcd_pow_coeffs: NULL output");
+    if (den != 0 && 2 * num == -den)                 // alpha = -1/2: the closed form
+        return qcd_inv_sqrt_coeffs(n, xmin, xmax, c0, coef, shift, delta);
+    const int rc = remez_pow(num, den, n, xmin, xmax, c0, coef, shift, delta);
+    if (rc == 1)
+        return fail(nullptr, QCD_EINVAL, "qcd_pow_coeffs: need 0 < |num/den| < 1, 1 <= n <= "
+                                         "QCD_MAX_SHIFTS and 0 < xmin < xmax");
+    if (rc != 0) return fail(nullptr, QCD_ENOTCONV, "qcd_pow_coeffs: the Remez iteration did not converge");
+    return QCD_OK;
+}
+
+qcd_status qcd_apply_pow(qcd_ctx *c, int parity, const double *d_phi, int num, int den, int n,
+                         double xmin, double xmax, double tol, int max_iter, double *d_out,
+                         int *iterations, double *true_res, double *delta)
+{
+    if (!c) return QCD_EINVAL;
+    if (!d_out || d_out == d_phi) return fail(c, QCD_EINVAL, "qcd_apply_pow: bad output pointer");
+    const qcd_ctx::PowFit *fit = nullptr;
+    for (const auto &f : c->pow_cache)
+        if (f.num == num && f.den == den && f.n == n && f.xmin == xmin && f.xmax == xmax) fit = &f;
+    if (!fit) {
+        qcd_ctx::PowFit f{num, den, n, xmin, xmax, 0.0, 0.0, {}, {}};
+        f.coef.resize(kMaxShifts); f.shift.resize(kMaxShifts);
+        const qcd_status s = qcd_pow_coeffs(num, den, n, xmin, xmax, &f.c0, f.coef.data(), f.shift.data(), &f.delta);
+        if (s != QCD_OK) return fail(c, s, qcd_last_error(nullptr));
+        if (c->pow_cache.size() >= 16) c->pow_cache.erase(c->pow_cache.begin());
+        c->pow_cache.push_back(std::move(f));
+        fit = &c->pow_cache.back();
+    }
+    if (delta) *delta = fit->delta;
+    return multishift_cg_impl(c, parity, d_phi, n, fit->shift.data(), fit->coef.data(), tol, max_iter,
+                              nullptr, d_out, iterations, true_res, true, fit->c0);
 }
 
 qcd_status qcd_inv_sqrt(qcd_ctx *c, int parity, const double *d_phi, int n, double xmin,

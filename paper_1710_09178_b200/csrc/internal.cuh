@@ -182,5 +182,8 @@ int launch_combine(long n2, const double2 *x, const long long *xoff_host, const 
 
 // host only (zolotarev.cu): minimax x^(-1/2) ~= c0 + sum_k c[k]/(x + d[k]) on [xmin, xmax]; 0 = ok
 int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, double *d, double *delta);
+// host only (remez.cu): minimax x^(num/den) ~= c0 + sum_k c[k]/(x + d[k]); 0 ok, 1 bad arguments, 2 not converged
+int remez_pow(int num, int den, int n, double xmin, double xmax, double *c0, double *c, double *d,
+              double *delta);
 
 }  // namespace qcd

@@ -56,32 +56,47 @@ struct Agm {
 
 }  // namespace
 
-// Returns 0, or 1 for bad arguments.  c and d hold n doubles each, d ascending.
-int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, double *d, double *delta)
+// The raw Zolotarev data for b = xmax/xmin and N = 2n+1, in the scaled variable y = x/xmin:
+//   a[l], l = 1..2n (a[0] unused):  a_l = sn^2/cn^2 (l K'/N)      -- poles (odd l) and zeros (even l) of r
+//   ref[j], j = 0..N:               y_j = 1/dn^2(j K'/N)          -- the 2n+2 equioscillation points
+// Returns 0, or 1 for bad arguments.
+int zolotarev_data(int n, double xmin, double xmax, double *a, double *ref)
 {
     if (n < 1 || n > kMaxShifts || !(xmin > 0.0) || !(xmax > xmin) || !std::isfinite(xmax)) return 1;
     const double b = xmax / xmin;
     const Agm agm(1.0 / b);
     const double Kp = agm.K();
     const int N = 2 * n + 1;
-    double a[2 * kMaxShifts + 2];                       // a[l], l = 1 .. 2n
     for (int l = 1; l <= n; ++l) {
         double p0, p1;
         agm.amplitude(l * Kp / N, p0, p1);
         const double t = std::tan(p0);
         a[l] = t * t;
+        if (ref) {
+            const double dn = std::cos(p0) / std::cos(p1 - p0);
+            ref[l] = 1.0 / (dn * dn);
+        }
     }
-    for (int l = n + 1; l <= 2 * n; ++l) a[l] = b / a[N - l];   // sn(K'-u) = cn(u)/dn(u)
+    for (int l = n + 1; l <= 2 * n; ++l) {
+        a[l] = b / a[N - l];                            // sn(K'-u) = cn(u)/dn(u)
+        if (ref) ref[l] = b / ref[N - l];               // dn(K'-u) = k/dn(u), k^2 = 1/b
+    }
+    if (ref) { ref[0] = 1.0; ref[N] = b; }
+    return 0;
+}
+
+// Returns 0, or 1 for bad arguments.  c and d hold n doubles each, d ascending.
+int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, double *d, double *delta)
+{
+    double a[2 * kMaxShifts + 2], ref[2 * kMaxShifts + 2];
+    if (zolotarev_data(n, xmin, xmax, a, ref) != 0) return 1;
     // den_k = a_{2k-1}, num_k = a_{2k}, k = 1..n
     auto f = [&](double y) {                            // sqrt(y) prod (y+num)/(y+den)
         double v = std::sqrt(y);
         for (int k = 1; k <= n; ++k) v *= (y + a[2 * k]) / (y + a[2 * k - 1]);
         return v;
     };
-    double p0, p1;
-    agm.amplitude(Kp / N, p0, p1);
-    const double dn1 = std::cos(p0) / std::cos(p1 - p0);
-    const double f0 = f(1.0), f1 = f(1.0 / (dn1 * dn1));
+    const double f0 = f(1.0), f1 = f(ref[1]);
     const double D = 2.0 / (f0 + f1);
     if (delta) *delta = std::fabs(f0 - f1) / (f0 + f1);
     // partial fractions in y, then x = xmin y:  1/sqrt(x) = r(y)/sqrt(xmin)

@@ -584,3 +584,35 @@ def test_config5_full_size(torch, q):
         assert tr <= 1.5 * cfg.tol and abs(tr - out["true_res"][k]) <= 1e-2 * tr
     assert rel_l2(out["y"], np.tensordot(res, out["x"], axes=(0, 0))) <= 1e-14
     _sampled_shift_check(rig, cfg, b, shifts, out, ks=(15,))
+
+
+# ------------------------------------------------------------------ (M^dag M)^(1/4) phi  (heat bath)
+
+def test_fourth_root_matches_oracle_and_dense_definition(torch, q):
+    """qcd_apply_pow with alpha = 1/4 on config 1: against eq. 8 with the ORACLE's Remez coefficients
+    and polished solves, against Q diag(lambda^(1/4)) Q^dag phi, and A^(1/4) A^(1/4) A^(-1/2) = 1."""
+    from fractions import Fraction
+    from oracle import rational as R
+    from helpers import c as cplx, dense_from_operator
+    cfg, links, b, _, _ = li.make_config_inputs(1)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    n, xmin, xmax = 10, 0.9 * cfg.mass ** 2, 8.5
+    d_phi, d_out = rig.to_internal(E, b), rig.ctx.new_vector()
+    st, it, tr, delta = rig.ctx.apply_pow(E, d_phi, 1, 4, n, xmin, xmax, 1e-11, 100000, d_out)
+    got = rig.to_canonical(E, d_out)
+    z = R.minimax_pow(Fraction(1, 4), n, xmin, xmax)
+    assert st == 0 and (tr <= 1.5e-11).all() and abs(delta / z["delta"] - 1) <= 1e-6
+    sol = rig.lat.solve_exact(cfg.mass, E, b, z["d"], z["c"], 1e-11)
+    assert rel_l2(got, z["c0"] * b + sol["y"]) <= TOL_X
+    a = dense_from_operator(lambda v: rig.lat.mdagm(cfg.mass, E, v), rig.nh)
+    lam, qm = np.linalg.eigh(a)
+    phi = cplx(b).reshape(-1)
+    exact = qm @ ((qm.conj().T @ phi) * lam ** 0.25)
+    assert np.linalg.norm(cplx(got).reshape(-1) - exact) / np.linalg.norm(exact) <= 1.05 * delta + 1e-9
+    # A^(1/4) A^(1/4) A^(-1/2) phi = phi
+    d_2, d_3 = rig.ctx.new_vector(), rig.ctx.new_vector()
+    rig.ctx.apply_pow(E, d_out, 1, 4, n, xmin, xmax, 1e-11, 100000, d_2)
+    _, _, _, delta_is = rig.ctx.inv_sqrt(E, d_2, n, xmin, xmax, 1e-11, 100000, d_3)
+    assert rel_l2(rig.to_canonical(E, d_3), b) <= 2.2 * delta + 1.1 * delta_is + 1e-8
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rig.ctx.apply_pow(E, d_phi, 5, 4, n, xmin, xmax, 1e-11, 100, d_out)

@@ -145,6 +145,15 @@ def test_minimax_pow_reproduces_the_closed_form_at_minus_one_half():
     assert np.abs(z["c"] / zz["c"] - 1).max() < 1e-13 and np.abs(z["d"] / zz["d"] - 1).max() < 1e-13
 
 
+def test_paper_degree_24_fourth_root_is_below_1e_12():
+    """The one number the paper prints about its coefficients (appendix): for ma =
+    0.005, xmin = 5e-5, xmax = 34 and 24 terms the x^(1/4) fit 'has an error of < 1e-12 throughout the
+    approximation range'.  A minimax error above that would contradict the paper; one far below it
+    would mean the oracle is not solving the paper's problem."""
+    z = R.minimax_pow(Fraction(1, 4), 24, 5e-5, 34.0, steps=3)
+    assert 1e-14 < z["delta"] < 1e-12
+
+
 def test_minimax_pow_fourth_power_and_inverse():
     z = R.minimax_pow(Fraction(1, 4), 9, 1e-4, 8.5)
     x = np.logspace(-4, np.log10(8.5), 499)

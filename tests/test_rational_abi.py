@@ -53,3 +53,54 @@ def test_bad_arguments():
     with pytest.raises(q.QcdError, match="QCD_EINVAL"):
         q.inv_sqrt_coeffs(3, 5.0, 1.0)
     assert lib.qcd_inv_sqrt(None, 0, None, 4, 1.0, 2.0, 1e-10, 10, None, None, None, None) == binding.QCD_EINVAL
+
+
+# ------------------------------------------------------------------ qcd_pow_coeffs (any exponent; x^(1/4))
+
+from fractions import Fraction  # noqa: E402
+
+POW_CASES = [(1, 4, 6, 1e-3, 7.0), (1, 4, 10, 2.5e-5, 8.5), (-1, 4, 9, 1e-4, 8.5), (1, 2, 8, 1e-4, 8.5),
+             (3, 4, 5, 1e-2, 9.0), (-1, 3, 7, 1e-3, 8.5)]
+
+
+@pytest.mark.parametrize("num,den,n,xmin,xmax", POW_CASES)
+def test_pow_coefficients_match_the_oracle(num, den, n, xmin, xmax):
+    """Library: Remez in binary128 (csrc/remez.cu).  Oracle: Remez in 50 digits with mpmath.  Both
+    stop when the extrema are level to ~1e-11 relative, which moves a coefficient by far less than
+    the 1e-9 asked here."""
+    c0, c, d, delta = q.pow_coeffs(num, den, n, xmin, xmax)
+    z = R.minimax_pow(Fraction(num, den), n, xmin, xmax)
+    assert abs(c0 / z["c0"] - 1) <= 1e-9
+    assert np.abs(c / z["c"] - 1).max() <= 1e-9 and np.abs(d / z["d"] - 1).max() <= 1e-9
+    assert abs(delta / z["delta"] - 1) <= 1e-6
+    assert (np.diff(d) > 0).all() and (d > 0).all() and (np.sign(c) == -np.sign(num)).all()
+
+
+def test_pow_library_meets_its_own_delta_and_the_papers_figure():
+    """x^(1/4) on [5e-5, 34] with 24 terms 'has an error of < 1e-12 throughout the
+    approximation range'.  The library's fit, evaluated in 50 digits, must say the same."""
+    c0, c, d, delta = q.pow_coeffs(1, 4, 24, 5e-5, 34.0)
+    assert 1e-14 < delta < 1e-12
+    x = 5e-5 * (34.0 / 5e-5) ** (np.arange(1501) / 1500.0)
+    err = R.relative_error_curve_pow(0.25, c0, c, d, x)
+    assert np.abs(err).max() <= delta * (1 + 1e-6) + 3e-15       # + rounding of 49 coefficients to double
+    assert np.abs(err).max() >= 0.99 * delta
+    # 'about 30 coefficients to achieve an error below 1e-11' at xmin < (2 m a)^2 = 1.6e-5 (PAPER.md:136)
+    assert q.pow_coeffs(1, 4, 30, 1.6e-5, 34.0)[3] < 1e-11
+
+
+def test_pow_minus_one_half_is_the_closed_form():
+    a = q.pow_coeffs(-1, 2, 12, 2.5e-5, 8.5)
+    b = q.inv_sqrt_coeffs(12, 2.5e-5, 8.5)
+    assert a[0] == b[0] and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    # and -2/4 is the same exponent
+    assert q.pow_coeffs(-2, 4, 12, 2.5e-5, 8.5)[0] == b[0]
+
+
+def test_pow_bad_arguments_and_over_resolution():
+    for num, den, n, lo, hi in ((0, 4, 4, 1.0, 2.0), (1, 0, 4, 1.0, 2.0), (4, 4, 4, 1.0, 2.0), (-5, 4, 4, 1.0, 2.0),
+                                (1, 4, 0, 1.0, 2.0), (1, 4, 65, 1.0, 2.0), (1, 4, 4, 2.0, 1.0), (1, 4, 4, 0.0, 1.0)):
+        with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+            q.pow_coeffs(num, den, n, lo, hi)
+    with pytest.raises(q.QcdError, match="QCD_ENOTCONV"):       # delta would be ~1e-40: nothing to level
+        q.pow_coeffs(1, 4, 40, 0.1, 8.5)
