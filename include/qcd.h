@@ -99,8 +99,10 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     (384 V bytes): "one often stores and moves only two rows ... of the (3 x 3)
  *                     complex link matrix and recovers the third by orthogonalization";
  *                     the stencil rebuilds row_2 = conj(row_0 x row_1) in registers.  REQUIRES links in
- *                     SU(3) (unitary, det = 1): rows 2 of the input are ignored.  Results differ from
- *                     the 3-row path at rounding level only (relative 1e-15) for SU(3) input.
+ *                     SU(3) (unitary, det = 1): qcd_load_gauge then checks every third row against
+ *                     conj(row_0 x row_1) (tolerance 1e-10 per component), SYNCHRONISES to read the
+ *                     verdict and returns QCD_EINVAL (no field loaded) if a link fails.  Results differ
+ *                     from the 3-row path at rounding level only (relative 1e-15).
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
        QCD_OPT_L2_PERSIST_MB = 5 };

@@ -390,10 +390,21 @@ qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
 {
     if (!c) return QCD_EINVAL;
     if (!d_links) return fail(c, QCD_EINVAL, "qcd_load_gauge: NULL links");
-    c->launches += launch_ingest_links(c->g, d_links, c->W, c->opt_link_rows, c->L());
+    int *flag = &c->st->not_su3;
+    QCD_CUDA(c, cudaMemsetAsync(flag, 0, sizeof(int), c->stream));
+    c->gauge_loaded = false;
+    c->launches += launch_ingest_links(c->g, d_links, c->W, c->opt_link_rows, flag, c->L());
     qcd_status s = check_launch(c, "qcd_load_gauge");
-    if (s == QCD_OK) { c->gauge_loaded = true; c->link_rows = c->opt_link_rows; setup_l2_window(c); }
-    return s;
+    if (s != QCD_OK) return s;
+    if (c->opt_link_rows == 2) {        // the one case in which this call synchronises (see qcd.h)
+        QCD_CUDA(c, cudaMemcpyAsync(&c->h_done[0], flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->h_done[0])
+            return fail(c, QCD_EINVAL, "qcd_load_gauge: two-row storage needs links in SU(3); a third row "
+                                       "differs from conj(row0 x row1) by more than 1e-10");
+    }
+    c->gauge_loaded = true; c->link_rows = c->opt_link_rows; setup_l2_window(c);
+    return QCD_OK;
 }
 
 qcd_status qcd_load_gauge_host(qcd_ctx *c, const double *h_links)

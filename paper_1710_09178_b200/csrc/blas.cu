@@ -39,6 +39,10 @@ cg_init_kernel(long n2, const double2 *__restrict__ b, double2 *__restrict__ r,
 }
 
 // r -= alpha q ; rho' = <r,r> ; last block: beta, beta_k, zeta rotation, freezing, stop test
+// LOOP: the kernel is a node of the WHILE graph of QCD_OPT_CG_GRAPH = 2 and sets its condition.  A
+// separate instantiation, because a kernel that references the device-side graph API is invisible to
+// ncu (the launch list of the default path would lose its r-update rows).
+template <bool LOOP>
 __global__ void __launch_bounds__(kBlock)
 cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q, double *partial,
                    CgState *st, cudaGraphConditionalHandle loop)
@@ -48,7 +52,7 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
     if (st->done) {                       // dead iteration after convergence
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             st->done_prev = 1;
-            if (loop) cudaGraphSetConditional(loop, 0);
+            if (LOOP) cudaGraphSetConditional(loop, 0);
         }
         return;
     }
@@ -67,7 +71,7 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
         cg_step_beta(st, total);
         // device-side loop (QCD_OPT_CG_GRAPH = 2): this iteration's shift update still runs (it is part
         // of the loop body); the WHILE node then stops when the stop test above has set `done`
-        if (loop && threadIdx.x == 0) cudaGraphSetConditional(loop, st->done ? 0u : 1u);
+        if (LOOP && threadIdx.x == 0) cudaGraphSetConditional(loop, st->done ? 0u : 1u);
     }
 }
 
@@ -175,8 +179,12 @@ int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstri
 int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
                        unsigned long long loop_handle, Launch L)
 {
-    launch_kernel(cg_update_r_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st,
-                  (cudaGraphConditionalHandle)loop_handle);
+    if (loop_handle)
+        launch_kernel(cg_update_r_kernel<true>, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st,
+                      (cudaGraphConditionalHandle)loop_handle);
+    else
+        launch_kernel(cg_update_r_kernel<false>, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st,
+                      (cudaGraphConditionalHandle)0);
     return 1;
 }
 

@@ -61,6 +61,7 @@ struct CgState {
     int done_prev;                // set one (dead) iteration later: gates the shift update
     unsigned counter;             // last-block-done ticket
     double scratch;               // generic reduction result (norms for true residuals)
+    int not_su3;                  // set by the two-row gauge ingest (layout.cu)
 };
 
 // ---- programmatic dependent launch (PDL) ----
@@ -120,7 +121,9 @@ struct Launch {
     const cudaAccessPolicyWindow *apw = nullptr;   // only the Dslash launches use it
 };
 
-int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, Launch L);
+// not_su3 (device int, zeroed by the caller): set to 1 by the two-row ingest when a link is not in SU(3)
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, int *not_su3,
+                        Launch L);
 // sites h0 <= h < h1 only (h1 < 0: all)
 int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L, int h0 = 0, int h1 = -1);
 int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L, int h0 = 0, int h1 = -1);

@@ -17,7 +17,7 @@ constexpr int kBlock = 256;
 // bit for bit ("stores and moves only two rows"); dslash.cu rebuilds the rest.
 template <int ROWS>
 __global__ void __launch_bounds__(kBlock)
-ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__ W)
+ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__ W, int *not_su3)
 {
     pdl_wait();
     pdl_launch_dependents();
@@ -47,6 +47,19 @@ ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__
             double2 v = u[c];
             w[(long)c * Vh] = make_double2(f * v.x, f * v.y);
         }
+        if (ROWS == 2) {
+            // two-row storage can only represent SU(3): refuse anything whose third row is not
+            // conj(row_0 x row_1) (qcd_load_gauge reports it; "recovers the third by
+            // orthogonalization" presupposes it)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const int c1 = (c + 1) % 3, c2 = (c + 2) % 3;
+                const double2 a1 = u[c1], a2 = u[c2], b1 = u[3 + c1], b2 = u[3 + c2], r = u[6 + c];
+                const double tx = a1.x * b2.x - a1.y * b2.y - a2.x * b1.x + a2.y * b1.y;
+                const double ty = a1.x * b2.y + a1.y * b2.x - a2.x * b1.y - a2.y * b1.x;
+                if (!(fabs(r.x - tx) <= 1e-10 && fabs(r.y + ty) <= 1e-10)) *not_su3 = 1;
+            }
+        }
     }
 }
 
@@ -75,13 +88,14 @@ unpack_kernel(int Vh, int h0, int h1, const double2 *__restrict__ v, double2 *__
 
 }  // namespace
 
-int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, Launch L)
+int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, int *not_su3,
+                        Launch L)
 {
     int blocks = (2 * g.Vh + kBlock - 1) / kBlock;
     if (link_rows == 2)
-        launch_kernel(ingest_links_kernel<2>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W);
+        launch_kernel(ingest_links_kernel<2>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W, not_su3);
     else
-        launch_kernel(ingest_links_kernel<3>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W);
+        launch_kernel(ingest_links_kernel<3>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W, not_su3);
     return 1;
 }
 

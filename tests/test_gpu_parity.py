@@ -164,17 +164,26 @@ def test_two_row_dslash_and_mdagm_match_oracle(torch, q, dims, kind):
         assert rel_l2(rig.mdagm(O, vo), lat.mdagm(0.07, O, vo)) <= TOL_OP
 
 
-def test_two_row_ignores_the_stored_third_row(torch, q):
-    """Only rows 0 and 1 are read: garbage in row 2 of the input changes nothing."""
+def test_two_row_refuses_links_outside_su3(torch, q):
+    """Two-row storage can only represent SU(3): a field whose third row is not conj(row0 x row1)
+    (here: one link out of 4*V scaled by 1 + 1e-6) is refused at load, loudly, and leaves the
+    context without a gauge field; the same field loads fine with three rows."""
     dims = (4, 6, 4, 4)
     links = li.make_links(dims, "random", 21)
     bad = links.reshape(-1, 4, 3, 3, 2).copy()
-    bad[:, :, 2] = 7.25
-    a = Rig(torch, q, dims, 0.1, links, link_rows=2)
-    b = Rig(torch, q, dims, 0.1, bad.reshape(links.shape), link_rows=2)
+    bad[137, 2, 2] *= 1.0 + 1e-6
+    bad = np.ascontiguousarray(bad.reshape(links.shape))
+    rig = Rig(torch, q, dims, 0.1, links, link_rows=2)
     v = li.make_source(dims, 3, E)
-    assert np.array_equal(a.dslash(O, v), b.dslash(O, v))
-    assert rel_l2(b.dslash(O, v), a.lat.dslash(O, v)) <= TOL_OP
+    good = rig.dslash(O, v)
+    with pytest.raises(q.QcdError, match="SU"):
+        rig.ctx.load_gauge(torch.from_numpy(bad).cuda())
+    with pytest.raises(q.QcdError, match="QCD_ESTATE"):
+        rig.dslash(O, v)
+    rig.ctx.load_gauge(rig.d_links)                       # a good field restores the context
+    assert np.array_equal(rig.dslash(O, v), good)
+    rig3 = Rig(torch, q, dims, 0.1, bad)                  # three-row storage takes any 3x3 matrices
+    assert rel_l2(rig3.dslash(O, v), rig3.lat.dslash(O, v)) <= TOL_OP
 
 
 def test_two_row_option_is_per_load_and_validated(torch, q):
