@@ -104,3 +104,36 @@ def test_pow_bad_arguments_and_over_resolution():
             q.pow_coeffs(num, den, n, lo, hi)
     with pytest.raises(q.QcdError, match="QCD_ENOTCONV"):       # delta would be ~1e-40: nothing to level
         q.pow_coeffs(1, 4, 40, 0.1, 8.5)
+
+
+def _golden_cases():
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "rational_coefficients.txt")
+    cases, cur = [], None
+    for line in open(path):
+        f = line.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] == "case":
+            cur = dict(num=int(f[1]), den=int(f[2]), n=int(f[3]), xmin=float(f[4]), xmax=float(f[5]),
+                       delta=float(f[6]), c0=float(f[7]), c=[], d=[])
+            cases.append(cur)
+        else:
+            cur["c"].append(float(f[1]))
+            cur["d"].append(float(f[2]))
+    return cases
+
+
+def test_library_against_the_stored_oracle_coefficients():
+    """tests/golden/rational_coefficients.txt is written by the oracle alone; the library must
+    reproduce every stored coefficient (and the oracle must still produce them: a regression pin)."""
+    cases = _golden_cases()
+    assert len(cases) == 4
+    for g in cases:
+        c0, c, d, delta = q.pow_coeffs(g["num"], g["den"], g["n"], g["xmin"], g["xmax"])
+        assert abs(c0 / g["c0"] - 1) <= 1e-9 and abs(delta / g["delta"] - 1) <= 1e-6
+        assert np.abs(c / np.array(g["c"]) - 1).max() <= 1e-9
+        assert np.abs(d / np.array(g["d"]) - 1).max() <= 1e-9
+    g = cases[0]
+    z = R.zolotarev_inv_sqrt(g["n"], g["xmin"], g["xmax"])
+    assert z["c0"] == g["c0"] and np.array_equal(z["c"], g["c"]) and np.array_equal(z["d"], g["d"])
