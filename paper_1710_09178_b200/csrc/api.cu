@@ -70,7 +70,10 @@ struct qcd_ctx {
     bool apw_on = false;
     long opt_l2_persist_mb = 0;         // QCD_OPT_L2_PERSIST_MB
     Launch L() const { return Launch{stream, opt_pdl, nullptr}; }
-    Launch Ld() const { return Launch{stream, opt_pdl, apw_on ? &apw : nullptr}; }
+    // Dslash launches: they read links before their PDL wait, so the first one after a gauge load must
+    // be fully serialised behind the ingest kernel
+    bool fresh_gauge = false;
+    Launch Ld() { const bool pdl = opt_pdl && !fresh_gauge; fresh_gauge = false; return Launch{stream, pdl, apw_on ? &apw : nullptr}; }
 };
 
 static std::string g_create_err;
@@ -404,6 +407,7 @@ qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
                                        "differs from conj(row0 x row1) by more than 1e-10");
     }
     c->gauge_loaded = true; c->link_rows = c->opt_link_rows; setup_l2_window(c);
+    c->fresh_gauge = true;
     return QCD_OK;
 }
 

@@ -20,6 +20,10 @@ constexpr int kBlock = kDslashBlock;
 #ifndef QCD_DSLASH3_MINB
 #define QCD_DSLASH3_MINB 4   // 128 registers: 24.4 / 120.5 / 393 us; unbounded (60 regs) 26.0 / 129 / 404; 1 (254 regs) 25.7 / 120.2 / 394
 #endif
+// link matrices requested before griddepcontrol.wait, in hop order +0, -0, +1, -1, ...
+#ifndef QCD_DSLASH_PREFETCH
+#define QCD_DSLASH_PREFETCH 2   // measured at 32^3x8: 0 -> 24.6 us, 1 -> 23.6, 2 -> 23.0, 3 (spills) -> 25.5
+#endif
 // minimum resident CTAs per SM asked of ptxas for the two-row kernel (caps its registers)
 #ifndef QCD_DSLASH2_MINB
 #define QCD_DSLASH2_MINB 4   // measured on B200 (32^3x8 / 48^3x12 / 64^3x16): 4 -> 16.8 / 83.4 / 274 us; 7 -> 17.1 / 88.6 / 276; 1 -> 18.9 / - / 296
@@ -42,7 +46,20 @@ dslash_kernel(const Geom g, const DslashParams p)
     const int par = p.out_parity;
     const int *hp = site.hp, *hm = site.hm, *nf = site.nf, *nb = site.nb;
     double dot = 0.0;
-    // everything above is index arithmetic; from here on data of the preceding kernel is read
+    // The gauge links are constant between qcd_load_gauge calls (and the first Dslash after a load is
+    // launched without PDL, api.cu), so the links of the first hops may be requested BEFORE waiting for
+    // the preceding kernel: they stream in while that kernel drains.
+    constexpr int NPF = QCD_DSLASH_PREFETCH;       // hops 0 .. NPF-1 in the order (+0, -0, +1, -1, ...)
+    double2 pre[NPF > 0 ? NPF : 1][9];
+    if (valid) {
+#pragma unroll
+        for (int k = 0; k < NPF; ++k) {
+            const int mu = k >> 1;
+            if (k & 1) load_link<ROWS>(p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
+            else load_link<ROWS>(p.W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
+        }
+    }
+    // everything above is index arithmetic and constant data; from here on data of the preceding kernel is read
     pdl_wait();
     pdl_launch_dependents();
     if (p.st != nullptr && p.st->done) return;   // CG already converged: dead iteration
@@ -55,7 +72,12 @@ dslash_kernel(const Geom g, const DslashParams p)
             {   // forward hop: + W_mu(x) in(x+mu), link based at x (parity par)
                 const double2 *__restrict__ w = p.W + ((long)(par * 4 + mu) * NW) * Vh + h;
                 double2 u[9], v[3];
-                load_link<ROWS>(w, Vh, u);
+                if (2 * mu < NPF) {
+#pragma unroll
+                    for (int i = 0; i < 9; ++i) u[i] = pre[2 * mu < NPF ? 2 * mu : 0][i];
+                } else {
+                    load_link<ROWS>(w, Vh, u);
+                }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hp[mu]);
                 if (ROWS == 2) {
@@ -70,7 +92,12 @@ dslash_kernel(const Geom g, const DslashParams p)
             {   // backward hop: - W_mu(x-mu)^dag in(x-mu), link based at x-mu (parity 1-par)
                 const double2 *__restrict__ w = p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu];
                 double2 u[9], v[3];
-                load_link<ROWS>(w, Vh, u);
+                if (2 * mu + 1 < NPF) {
+#pragma unroll
+                    for (int i = 0; i < 9; ++i) u[i] = pre[2 * mu + 1 < NPF ? 2 * mu + 1 : 0][i];
+                } else {
+                    load_link<ROWS>(w, Vh, u);
+                }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hm[mu]);
                 if (ROWS == 2) {

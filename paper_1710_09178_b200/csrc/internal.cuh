@@ -70,7 +70,9 @@ struct CgState {
 // (or graph) is still draining, runs its index arithmetic, and blocks in pdl_wait() until the
 // predecessor has completed and its writes are visible.  Rules kept by every kernel: nothing written
 // and nothing produced by an earlier kernel read before pdl_wait(); pdl_launch_dependents() only
-// after pdl_wait(), so completion is transitive along the chain.
+// after pdl_wait(), so completion is transitive along the chain.  One deliberate use of the window:
+// the Dslash requests its first two link matrices BEFORE pdl_wait() -- the gauge field is constant
+// between qcd_load_gauge calls, and the first Dslash after a load is launched without PDL (api.cu).
 #ifdef __CUDACC__
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents()
