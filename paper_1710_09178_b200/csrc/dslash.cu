@@ -51,18 +51,24 @@ dslash_kernel(const Geom g, const DslashParams p)
     // the preceding kernel: they stream in while that kernel drains.
     constexpr int NPF = QCD_DSLASH_PREFETCH;       // hops 0 .. NPF-1 in the order (+0, -0, +1, -1, ...)
     double2 pre[NPF > 0 ? NPF : 1][9];
-    if (valid) {
+    auto request_links = [&]() {
 #pragma unroll
         for (int k = 0; k < NPF; ++k) {
             const int mu = k >> 1;
             if (k & 1) load_link<ROWS>(p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
             else load_link<ROWS>(p.W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
         }
-    }
+    };
+    // Inside the CG, `done` was last written two or more kernels back (r-update), which has completed
+    // by the time this kernel may start: a dead iteration is recognised early and requests nothing.
+    // (Only a hint: after a cg_init for a zero source it may still read 0; the check after the wait decides.)
+    const bool early = valid && !(p.st != nullptr && *(volatile const int *)&p.st->done);
+    if (early) request_links();
     // everything above is index arithmetic and constant data; from here on data of the preceding kernel is read
     pdl_wait();
     pdl_launch_dependents();
     if (p.st != nullptr && p.st->done) return;   // CG already converged: dead iteration
+    if (valid && !early) request_links();
     if (valid) {
         const double2 *__restrict__ in = p.in;
         double2 acc[3];
