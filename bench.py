@@ -48,7 +48,7 @@ FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
 # summarised in profiles/ (None until a capture for that workload exists).
 # key: (config number, link rows)
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 163.65e6, (3, 2): 110.99e6,   # profiles/r01_dslash_full_cfg3.md
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 162.98e6, (3, 2): 111.49e6,   # profiles/r01_dslash_full_cfg3.md
                              (5, 3): 2.665e9}                       # profiles/r01_dslash_full_cfg5.md
 
 
