@@ -461,6 +461,20 @@ def main():
                                    "what": "qcd_apply_pow(1/4): Remez coefficients in binary128 on the "
                                            "first call, then one multishift CG + fused combine"}
 
+            # QCD_OPT_Y_ONLY: the same two applications without forming the x_k
+            ctx.set_option(q.QCD_OPT_Y_ONLY, 1)
+            for key, fn in (("inv_sqrt", lambda: ctx.inv_sqrt(cfg.parity, d_b, cfg.nshift, xmin, xmax, cfg.tol, 100000, d_y)),
+                            ("fourth_root", lambda: ctx.apply_pow(cfg.parity, d_b, 1, 4, cfg.nshift, xmin, xmax, cfg.tol, 100000, d_y))):
+                ts = []
+                for _ in range(3):
+                    torch.cuda.synchronize()
+                    w0 = time.perf_counter()
+                    st, it, tr, delta = fn()
+                    ts.append(time.perf_counter() - w0)
+                    assert st == 0 and tr.max() <= 1.5 * cfg.tol, (st, tr)
+                line[key]["y_only_s_per_apply"] = statistics.median(ts[1:])
+            ctx.set_option(q.QCD_OPT_Y_ONLY, 0)
+
         if R == 3 and not args.no_two_row:
             # the same sections A and C with two-row link storage
             ctx.set_option(q.QCD_OPT_LINK_ROWS, 2)

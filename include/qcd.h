@@ -94,6 +94,13 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     persisting set-aside of L2 (capped by the device limits; the limit is device-
  *                     wide).  Helps back-to-back applies on lattices slightly larger than L2, hurts the
  *                     CG when the set-aside takes L2 away from its vectors.  Bit-identical results.
+ *   QCD_OPT_Y_ONLY    (default 0) qcd_inv_sqrt and qcd_apply_pow need only y = c0 phi + sum c_k x_k, so with
+ *                     1 the shifted solutions x_k are never formed: the iteration accumulates
+ *                     y += c_k alpha_k p_k directly, which halves the traffic of the per-shift update
+ *                     and skips the residual pass.  y agrees with the default path to rounding.
+ *                     true_res[] then holds the recursion's ESTIMATES |zeta_k| sqrt(rho)/||b|| (the
+ *                     freezing threshold 0.1 tol for shifts frozen early), not recomputed residuals.
+ *                     qcd_multishift_cg is not affected.
  *   QCD_OPT_LINK_ROWS (default 3) how the NEXT qcd_load_gauge stores the links.  3: all nine entries
  *                     (576 V bytes, "72V double precision words").  2: two-row storage
  *                     (384 V bytes): "one often stores and moves only two rows ... of the (3 x 3)
@@ -105,7 +112,7 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     from the 3-row path at rounding level only (relative 1e-15).
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
-       QCD_OPT_L2_PERSIST_MB = 5 };
+       QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

@@ -53,15 +53,16 @@ struct qcd_ctx {
     bool opt_pdl = true;                // programmatic dependent launch on every kernel
     int opt_cg_graph = 1;               // 0: plain launches; 1: one captured graph per batch; 2: device-side WHILE loop
     unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
+    bool opt_y_only = false;            // qcd_inv_sqrt / qcd_apply_pow accumulate y directly, no x_k
     int opt_cg_batch = 8;               // iterations enqueued per batch / per graph
     // cached graph of one batch of CG iterations (valid for exactly the key below)
     cudaGraphExec_t cg_exec = nullptr;
     cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
     struct CgKey {
-        int parity = -1, batch = 0, rows = 0; bool pdl = false, apw = false; double mass = 0.0;
+        int parity = -1, batch = 0, rows = 0; bool pdl = false, apw = false, yonly = false; double mass = 0.0;
         const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
         bool operator==(const CgKey &o) const {
-            return parity == o.parity && batch == o.batch && rows == o.rows && pdl == o.pdl && apw == o.apw && mass == o.mass &&
+            return parity == o.parity && batch == o.batch && rows == o.rows && pdl == o.pdl && apw == o.apw && yonly == o.yonly && mass == o.mass &&
                    x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
         }
     } cg_key;
@@ -179,21 +180,24 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
 }
 
 // one multishift-CG iteration: 4 kernels, all scalars stay on the device
-void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x)
+void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
 {
     // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
     run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
     run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
     c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->partial, c->st, c->loop_handle, c->L());
-    c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
+    if (y_only)      // `x` is the single vector y
+        c->launches += launch_cg_update_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
+    else
+        c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
 }
 
 // Capture `batch` iterations into a graph (once per distinct set of buffers, parity and mass);
 // batch == 0: the device-side loop graph.
-qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
+qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y_only)
 {
     qcd_ctx::CgKey key;
-    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.mass = c->mass;
+    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
     key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp;
     if (c->cg_exec && key == c->cg_key) return QCD_OK;
     if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }
@@ -206,7 +210,7 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
     if (batch > 0) {
         e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
         if (e == cudaSuccess) {
-            for (int i = 0; i < batch; ++i) enqueue_cg_iteration(c, parity, x);
+            for (int i = 0; i < batch; ++i) enqueue_cg_iteration(c, parity, x, y_only);
             cudaGraph_t graph = nullptr;
             e = cudaStreamEndCapture(c->cap_stream, &graph);
             if (e == cudaSuccess) e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
@@ -232,7 +236,7 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch)
             e = cudaStreamBeginCaptureToGraph(c->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
             if (e == cudaSuccess) {
                 c->loop_handle = (unsigned long long)handle;
-                enqueue_cg_iteration(c, parity, x);
+                enqueue_cg_iteration(c, parity, x, y_only);
                 c->loop_handle = 0;
                 cudaGraph_t same = nullptr;
                 e = cudaStreamEndCapture(c->cap_stream, &same);
@@ -373,6 +377,7 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         c->g.tgroup = value == 0 ? auto_tgroup(c->g) : value > c->g.chunks ? c->g.chunks : (int)value;
         if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }   // Geom is baked in
         return QCD_OK;
+    case QCD_OPT_Y_ONLY: c->opt_y_only = value != 0; return QCD_OK;
     case QCD_OPT_L2_PERSIST_MB:
         if (value < 0) return fail(c, QCD_EINVAL, "qcd_set_option: L2 persist size must be >= 0");
         c->opt_l2_persist_mb = value;
@@ -472,7 +477,7 @@ namespace {
 qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nshift,
                               const double *shifts, const double *residues, double tol,
                               int max_iter, double *d_x, double *d_y, int *iterations,
-                              double *true_res, bool with_c0, double c0)
+                              double *true_res, bool with_c0, double c0, bool y_only = false)
 {
     if (!c) return QCD_EINVAL;
     if (bad_parity(parity) || !d_b || !shifts || !residues || !iterations || !true_res)
@@ -484,13 +489,15 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     for (int k = 0; k < nshift; ++k)
         if (!(shifts[k] >= 0.0)) return fail(c, QCD_EINVAL, "qcd_multishift_cg: shifts must be >= 0");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_multishift_cg: no gauge field loaded");
-    qcd_status s = ensure_cg_workspace(c, nshift, d_x == nullptr);
+    y_only = y_only && d_x == nullptr && d_y != nullptr;
+    qcd_status s = ensure_cg_workspace(c, nshift, d_x == nullptr && !y_only);
     if (s != QCD_OK) return s;
 
     const long n2 = c->n2;
     cudaStream_t st = c->stream;
     const double2 *b = (const double2 *)d_b;
-    double2 *x = d_x ? (double2 *)d_x : c->xws;
+    // y-only: the "x buffer" of the iteration is the single accumulator y
+    double2 *x = y_only ? (double2 *)d_y : d_x ? (double2 *)d_x : c->xws;
 
     // base system = smallest shift (C12): sort, remember the caller's order
     std::vector<int> order(nshift);
@@ -510,20 +517,21 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         h.active[k] = 1;
         h.xoff[k] = (long long)(d_x ? order[k] : k) * n2;
         xoff_caller[order[k]] = h.xoff[k];
+        h.cy[k] = residues[order[k]];
     }
     h.sigma0 = h.sigma[0];
     QCD_CUDA(c, cudaMemcpyAsync(c->st, &h, sizeof h, cudaMemcpyHostToDevice, st));
-    QCD_CUDA(c, cudaMemsetAsync(x, 0, (size_t)n2 * nshift * sizeof(double2), st));
+    QCD_CUDA(c, cudaMemsetAsync(x, 0, (size_t)n2 * (y_only ? 1 : nshift) * sizeof(double2), st));
     c->launches += launch_cg_init(n2, b, c->r, c->p, n2, nshift, c->partial, c->st, c->L());
 
     // iteration loop: enqueue only (one graph replay, or 4 launches per iteration, per batch)
     const int batch = std::max(1, std::min(c->opt_cg_batch, max_iter));
     const bool use_graph = c->opt_cg_graph == 1;
     if (c->opt_cg_graph == 2) {
-        if ((s = ensure_cg_graph(c, parity, x, 0)) != QCD_OK) return s;
+        if ((s = ensure_cg_graph(c, parity, x, 0, y_only)) != QCD_OK) return s;
         QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));     // launch count added below, once iter is known
     } else {
-    if (use_graph && (s = ensure_cg_graph(c, parity, x, batch)) != QCD_OK) return s;
+    if (use_graph && (s = ensure_cg_graph(c, parity, x, batch, y_only)) != QCD_OK) return s;
     int enq = 0, cur = 0;
     bool pending = false, finished = false;
     c->h_done[0] = c->h_done[1] = 0;
@@ -534,7 +542,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
             QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));
             c->launches += 4L * batch;
         } else {
-            for (int i = 0; i < nb; ++i) enqueue_cg_iteration(c, parity, x);
+            for (int i = 0; i < nb; ++i) enqueue_cg_iteration(c, parity, x, y_only);
         }
         enq += nb;
         if (pending) {
@@ -550,7 +558,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
 
     // finish (a6): true residuals recomputed from x_k, kMultiRhs shifts per pass over the links;
     // the p_k are dead by now and serve as the tmp vectors.  y = sum_k c_k x_k.
-    for (int k0 = 0; k0 < nshift; k0 += kMultiRhs) {
+    for (int k0 = 0; k0 < (y_only ? 0 : nshift); k0 += kMultiRhs) {
         const int nb = std::min(kMultiRhs, nshift - k0);
         DslashMultiParams mp{};
         mp.W = c->W; mp.link_rows = c->link_rows; mp.nrhs = nb;
@@ -569,7 +577,13 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         }
         c->launches += launch_dslash_multi(c->g, mp, c->Ld());
     }
-    if (d_y)
+    if (y_only) {
+        if (with_c0) {      // y <- c0 b + 1 * y, in place (every thread reads its element before writing it)
+            const long long zero = 0;
+            const double one = 1.0;
+            c->launches += launch_combine(n2, x, &zero, &one, 1, c0, b, x, c->L());
+        }
+    } else if (d_y)
         c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, c0,
                                       with_c0 ? b : nullptr, (double2 *)d_y, c->L());
     s = check_launch(c, "qcd_multishift_cg");
@@ -583,6 +597,10 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     const double rho_b = h.rho_b;
     for (int k = 0; k < nshift; ++k)
         true_res[k] = rho_b > 0.0 ? std::sqrt(c->h_results[k] / rho_b) : 0.0;
+    if (y_only)      // no x_k to recompute from: the recursion's own estimate |zeta_k| sqrt(rho/rho_b),
+        for (int k = 0; k < nshift; ++k)        // and the freezing threshold for the frozen shifts
+            true_res[order[k]] = rho_b > 0.0 ? (h.active[k] ? std::fabs(h.zeta[k]) * std::sqrt(h.rho / rho_b)
+                                                            : h.freeze * tol) : 0.0;
     const bool converged = rho_b == 0.0 || std::sqrt(h.rho / rho_b) <= tol;
     if (!converged) return fail(c, QCD_ENOTCONV, "qcd_multishift_cg: max_iter reached");
     return QCD_OK;
@@ -646,7 +664,7 @@ qcd_status qcd_apply_pow(qcd_ctx *c, int parity, const double *d_phi, int num, i
     }
     if (delta) *delta = fit->delta;
     return multishift_cg_impl(c, parity, d_phi, n, fit->shift.data(), fit->coef.data(), tol, max_iter,
-                              nullptr, d_out, iterations, true_res, true, fit->c0);
+                              nullptr, d_out, iterations, true_res, true, fit->c0, c->opt_y_only);
 }
 
 qcd_status qcd_inv_sqrt(qcd_ctx *c, int parity, const double *d_phi, int n, double xmin,
@@ -659,7 +677,7 @@ qcd_status qcd_inv_sqrt(qcd_ctx *c, int parity, const double *d_phi, int n, doub
     if (zolotarev_inv_sqrt(n, xmin, xmax, &c0, coef, shift, delta) != 0)
         return fail(c, QCD_EINVAL, "qcd_inv_sqrt: need 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax");
     return multishift_cg_impl(c, parity, d_phi, n, shift, coef, tol, max_iter, nullptr, d_out,
-                              iterations, true_res, true, c0);
+                              iterations, true_res, true, c0, c->opt_y_only);
 }
 
 qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, double *h_out)

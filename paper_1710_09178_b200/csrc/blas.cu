@@ -132,6 +132,60 @@ cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restr
     }
 }
 
+// y-only form of the shift update (QCD_OPT_Y_ONLY): when only y = sum_k c_k x_k is wanted (eq. 8,
+// the heat bath and the action need (M^dag M)^(1/b) phi, not the x_k), the x_k never
+// have to exist: x_k += alpha_k p_k turns into y += c_k alpha_k p_k, accumulated in registers over the
+// active shifts of an element.  Per active shift the kernel then moves p_k in and out (48 V bytes)
+// instead of x_k and p_k (96 V bytes); r and y once per element.
+__global__ void __launch_bounds__(kBlock)
+cg_update_shifts_y_kernel(long n2, const double2 *__restrict__ r, double2 *__restrict__ y,
+                          double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    if (st->done_prev) return;
+    __shared__ double s_ca[kMaxShifts], s_z[kMaxShifts], s_b[kMaxShifts];
+    __shared__ long long s_p[kMaxShifts];
+    const int nl = st->nlist;
+    if (threadIdx.x < nl) {
+        const int k = st->list[threadIdx.x];
+        s_ca[threadIdx.x] = st->cy[k] * st->coef_a[k];
+        s_z[threadIdx.x] = st->coef_z[k];
+        s_b[threadIdx.x] = st->coef_b[k];
+        s_p[threadIdx.x] = (long long)k * pstride;
+    }
+    __syncthreads();
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        const double2 rv = __ldg(r + i);
+        double2 yv = y[i];
+        int j = 0;
+        for (; j + 1 < nl; j += 2) {                 // two shifts in flight per thread
+            double2 *pa = p + s_p[j] + i, *pb = p + s_p[j + 1] + i;
+            double2 va = *pa, vb = *pb;
+            yv.x = fma(s_ca[j], va.x, yv.x);
+            yv.y = fma(s_ca[j], va.y, yv.y);
+            yv.x = fma(s_ca[j + 1], vb.x, yv.x);
+            yv.y = fma(s_ca[j + 1], vb.y, yv.y);
+            va.x = fma(s_b[j], va.x, s_z[j] * rv.x);
+            va.y = fma(s_b[j], va.y, s_z[j] * rv.y);
+            vb.x = fma(s_b[j + 1], vb.x, s_z[j + 1] * rv.x);
+            vb.y = fma(s_b[j + 1], vb.y, s_z[j + 1] * rv.y);
+            *pa = va;
+            *pb = vb;
+        }
+        if (j < nl) {
+            double2 *pa = p + s_p[j] + i;
+            double2 va = *pa;
+            yv.x = fma(s_ca[j], va.x, yv.x);
+            yv.y = fma(s_ca[j], va.y, yv.y);
+            va.x = fma(s_b[j], va.x, s_z[j] * rv.x);
+            va.y = fma(s_b[j], va.y, s_z[j] * rv.y);
+            *pa = va;
+        }
+        y[i] = yv;
+    }
+}
+
 struct CombineArgs {
     long long xoff[kMaxShifts];
     double c[kMaxShifts];
@@ -195,6 +249,15 @@ int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, l
     long units = (n2 + kShiftChunk - 1) / kShiftChunk * kMaxShifts;
     int grid = (int)(units < 148 * 8 ? (units > 0 ? units : 1) : 148 * 8);
     launch_kernel(cg_update_shifts_kernel, grid, kBlock, L.s, L.pdl, n2, r, x, p, pstride, st);
+    return 1;
+}
+
+int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p, long pstride,
+                              CgState *st, Launch L)
+{
+    long blocks = (n2 + kBlock - 1) / kBlock;
+    int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
+    launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, r, y, p, pstride, st);
     return 1;
 }
 

@@ -62,6 +62,7 @@ struct CgState {
     unsigned counter;             // last-block-done ticket
     double scratch;               // generic reduction result (norms for true residuals)
     int not_su3;                  // set by the two-row gauge ingest (layout.cu)
+    double cy[kMaxShifts];        // y-only mode: residues c_k of eq. 8 in sorted-shift order
 };
 
 // ---- programmatic dependent launch (PDL) ----
@@ -179,6 +180,9 @@ int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstri
 // loop_handle != 0: the kernel is a node of a WHILE conditional graph and sets its condition
 int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
                        unsigned long long loop_handle, Launch L);
+// y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept)
+int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p, long pstride,
+                              CgState *st, Launch L);
 int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
                             CgState *st, Launch L);
 // y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)

@@ -625,3 +625,36 @@ def test_fourth_root_matches_oracle_and_dense_definition(torch, q):
     assert rel_l2(rig.to_canonical(E, d_3), b) <= 2.2 * delta + 1.1 * delta_is + 1e-8
     with pytest.raises(q.QcdError, match="QCD_EINVAL"):
         rig.ctx.apply_pow(E, d_phi, 5, 4, n, xmin, xmax, 1e-11, 100, d_out)
+
+
+@pytest.mark.parametrize("number,n", [(1, 10), (2, 12)])
+def test_y_only_mode_gives_the_same_y_without_forming_x(torch, q, number, n):
+    """QCD_OPT_Y_ONLY: qcd_inv_sqrt / qcd_apply_pow accumulate y += c_k alpha_k p_k in the iteration.
+    Same y as the default path to rounding, same y as the oracle's eq. 8; the reported residuals are
+    the recursion's estimates and must bracket the recomputed ones."""
+    from fractions import Fraction
+    from oracle import rational as R
+    cfg, links, b, _, _ = li.make_config_inputs(number)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    xmin, xmax, tol = 0.9 * cfg.mass ** 2, 8.5, 1e-11
+    d_phi, d_a, d_b = rig.to_internal(E, b), rig.ctx.new_vector(), rig.ctx.new_vector()
+    for num, den in ((-1, 2), (1, 4)):
+        rig.ctx.set_option(q.QCD_OPT_Y_ONLY, 0)
+        st0, it0, tr0, delta0 = rig.ctx.apply_pow(E, d_phi, num, den, n, xmin, xmax, tol, 100000, d_a)
+        rig.ctx.set_option(q.QCD_OPT_Y_ONLY, 1)
+        l0 = rig.ctx.launch_count
+        st1, it1, tr1, delta1 = rig.ctx.apply_pow(E, d_phi, num, den, n, xmin, xmax, tol, 100000, d_b)
+        ya, yb = rig.to_canonical(E, d_a), rig.to_canonical(E, d_b)
+        assert st0 == 0 and st1 == 0 and it0 == it1 and delta0 == delta1
+        assert rel_l2(yb, ya) <= 1e-12
+        z = (R.zolotarev_inv_sqrt(n, xmin, xmax) if (num, den) == (-1, 2)
+             else R.minimax_pow(Fraction(num, den), n, xmin, xmax))
+        sol = rig.lat.solve_exact(cfg.mass, E, b, z["d"], z["c"], tol)
+        assert rel_l2(yb, z["c0"] * b + sol["y"]) <= TOL_X
+        assert (tr1 <= 1.5 * tol).all() and (tr1 > 0).all()
+        assert (tr0 <= 1.5 * tol).all()
+        assert tr1[0] == pytest.approx(tr0[0], rel=0.05)          # base shift: recursion vs recomputed
+    # the inv_sqrt entry point takes the same path; the zero source still works
+    st, it, tr, _ = rig.ctx.inv_sqrt(E, torch.zeros_like(d_phi), n, xmin, xmax, tol, 100, d_b)
+    assert st == 0 and it == 0 and not rig.to_canonical(E, d_b).any() and not tr.any()
+    rig.ctx.set_option(q.QCD_OPT_Y_ONLY, 0)
