@@ -13,6 +13,9 @@ of applies):
     A. PAIRS x (D_oe, D_eo) back to back, one CUDA graph          (a2, a3)   -> `value`
     B. PAIRS/2 x M^dag M                                           (a4)
     C. one multishift-CG solve incl. true residuals and y         (a5, a6)   -> cg.s_per_solve
+After the timed region, once, on rank 0: the e2e leg (host buffers through the C ABI), (M^dag M)^(-1/2) phi and
+(M^dag M)^(1/4) phi via eq. 8 (`inv_sqrt`, `fourth_root`; also with QCD_OPT_Y_ONLY), the two-row-link
+variant of sections A and C (`two_row`), and the oracle on the host cores (`cpu_baseline`).
 `value` = 624*V bytes x (Dslash launches of section A) / (CUDA-event time of section A), summed over
 the K steps.  Inputs (151 MB of links + vectors) are larger than the 126 MB L2, so no explicit L2
 flush is issued between iterations; `roofline.traffic` gives the DRAM bytes ncu measured per launch.
