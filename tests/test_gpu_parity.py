@@ -658,3 +658,34 @@ def test_y_only_mode_gives_the_same_y_without_forming_x(torch, q, number, n):
     st, it, tr, _ = rig.ctx.inv_sqrt(E, torch.zeros_like(d_phi), n, xmin, xmax, tol, 100, d_b)
     assert st == 0 and it == 0 and not rig.to_canonical(E, d_b).any() and not tr.any()
     rig.ctx.set_option(q.QCD_OPT_Y_ONLY, 0)
+
+
+def test_random_shapes_rows_and_cta_orders(torch, q):
+    """A seeded sweep over lattice shapes (extents 2..16, odd half-extents, thin directions), both
+    link layouts and three CTA orders: Dslash and M^dag M element by element, a 5-shift solve against
+    independent single-shift oracle CGs."""
+    rng = np.random.default_rng(2024)
+    shapes = {(16, 2, 2, 2), (2, 16, 2, 2), (2, 2, 16, 2), (2, 2, 2, 16), (18, 14, 10, 6)}
+    while len(shapes) < 14:
+        d = tuple(int(2 * rng.integers(1, 9)) for _ in range(4))
+        if np.prod(d) <= 12000:
+            shapes.add(d)
+    mass = 0.13
+    shifts, res = np.array([0.7, 0.0, 0.05, 2.5, 0.3]), np.array([1.0, -0.5, 2.0, 0.25, 3.0])
+    for dims in sorted(shapes):
+        links = li.make_links(dims, "random", sum(dims))
+        for rows in (3, 2):
+            rig = Rig(torch, q, dims, mass, links, link_rows=rows)
+            for tg in (0, 1, 2):
+                rig.ctx.set_option(q.QCD_OPT_TGROUP, tg)
+                for par in (O, E):
+                    v, w = li.make_source(dims, 7 + par, 1 - par), li.make_source(dims, 9 + par, par)
+                    assert rel_l2(rig.dslash(par, v), rig.lat.dslash(par, v)) <= TOL_OP, (dims, rows, tg, par)
+                    assert rel_l2(rig.mdagm(par, w), rig.lat.mdagm(mass, par, w)) <= TOL_OP, (dims, rows, tg, par)
+            b = li.make_source(dims, 3, E)
+            out = rig.solve(E, b, shifts, res, 1e-11)
+            assert out["status"] == 0 and (out["true_res"] <= 1.5e-11).all(), (dims, rows)
+            for k in (1, 3):
+                xs, _, _, st = rig.lat.cg(mass, E, shifts[k], b, 1e-14, max_iter=20000)
+                assert st == 0 and rel_l2(out["x"][k], xs) <= TOL_X, (dims, rows, k)
+            rig.ctx.close()
