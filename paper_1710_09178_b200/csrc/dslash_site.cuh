@@ -122,7 +122,14 @@ template <int ROWS>
 __device__ __forceinline__ void load_link(const double2 *__restrict__ w, int Vh, double2 *u)
 {
 #pragma unroll
-    for (int i = 0; i < 3 * ROWS; ++i) u[i] = __ldg(w + (long)i * Vh);
+    // Links are used exactly once per apply: load them with the streaming (evict-first) policy, so that
+    // L2 keeps the vectors (the output of one Dslash is the gathered input of the next) and does not
+    // cycle the whole gauge field through LRU.  Measured, us per apply at 32^3x8 / 48^3x12 / 64^3x16:
+    // __ldg 22.9 / 120.7 / 379.3, __ldcs 21.1 / 117.8 / 376.3 (two-row at 32^3x8: 16.4 -> 15.5).
+#ifndef QCD_LINK_LOAD
+#define QCD_LINK_LOAD __ldcs
+#endif
+    for (int i = 0; i < 3 * ROWS; ++i) u[i] = QCD_LINK_LOAD(w + (long)i * Vh);
     if (ROWS == 2) third_row(u);
 }
 
