@@ -50,8 +50,10 @@ PAIRS = 50                      # (D_oe, D_eo) pairs per step in section A
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
 # summarised in profiles/ (None until a capture for that workload exists).
+# steady-state (no cache flush) DRAM read+write per launch, mean of D_oe and D_eo (profiles/r01_dslash_full_cfg3.md)
+NCU_WARM_DRAM_BYTES_PER_LAUNCH = {(3, 3): 128.9e6, (3, 2): 109.6e6}
 # key: (config number, link rows)
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 162.98e6, (3, 2): 111.49e6,   # profiles/r01_dslash_full_cfg3.md
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 161.07e6, (3, 2): 110.96e6,   # profiles/r01_dslash_full_cfg3.md
                              (5, 3): 2.665e9}                       # profiles/r01_dslash_full_cfg5.md
 
 
@@ -387,7 +389,11 @@ def main():
                      "peak_source": peak_src,
                      "peak_note": "hbm_gbs is a copy (read+write) rate; this kernel is 96 % reads, so frac "
                                   "can exceed 1 (read-only probe of the same pattern: DESIGN.md section 5)", "algorithmic_bytes_per_launch": dslash_bytes(V, R), "link_rows": R,
-                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((cfg.number, R))},
+                     "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((cfg.number, R)),
+                     "traffic_warm": NCU_WARM_DRAM_BYTES_PER_LAUNCH.get((cfg.number, R)),
+                     "traffic_note": "traffic: ncu --set full (cold L2, per launch); traffic_warm: same "
+                                     "kernel inside the graph replay without cache flush -- the output of one "
+                                     "apply and part of the links are served by L2 (profiles/)"},
         "gpu_launches": K * (launches_a + launches_b + cg_launches),
     }
     if not args.no_solve:
