@@ -48,11 +48,11 @@ METRIC = "staggered_dslash_fp64_algorithmic_GBps"
 UNIT = "GB/s"
 PAIRS = 50                      # (D_oe, D_eo) pairs per step in section A
 FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
-# summarised in profiles/ (None until a capture for that workload exists).
+# key of both tables: (config number, link rows)
 # steady-state (no cache flush) DRAM read+write per launch, mean of D_oe and D_eo (profiles/r01_dslash_full_cfg3.md)
 NCU_WARM_DRAM_BYTES_PER_LAUNCH = {(3, 3): 128.9e6, (3, 2): 109.6e6}
-# key: (config number, link rows)
+# dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch from the `ncu --set full` capture
+# summarised in profiles/ (absent until a capture for that workload exists)
 NCU_DRAM_BYTES_PER_LAUNCH = {(3, 3): 161.07e6, (3, 2): 110.96e6,   # profiles/r01_dslash_full_cfg3.md
                              (5, 3): 2.665e9}                       # profiles/r01_dslash_full_cfg5.md
 
