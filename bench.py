@@ -396,6 +396,39 @@ def main():
                                      "apply and part of the links are served by L2 (profiles/)"},
         "gpu_launches": K * (launches_a + launches_b + cg_launches),
     }
+    # the same apply with a COLD L2: a 512 MB buffer is overwritten before every single launch, no graph,
+    # no PDL overlap with a predecessor -- what one isolated Dslash costs (section A above is the steady
+    # state of back-to-back applies, where L2 holds the vectors and part of the links)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    cold = []
+    for i in range(12):
+        flush.fill_(i & 0xFF)
+        e0, e1 = ev(), ev()
+        e0.record()
+        ctx.dslash(1 - (i & 1), d_b if not (i & 1) else d_o, d_o if not (i & 1) else d_e)
+        e1.record()
+        torch.cuda.synchronize()
+        cold.append(e0.elapsed_time(e1) * 1e-3)
+    empty = []                               # what the event bracket itself costs around a trivial kernel
+    tiny = flush[:128]
+    for i in range(12):
+        flush.fill_(i & 0xFF)                # keeps the GPU busy while the host enqueues the bracket
+        e0, e1 = ev(), ev()
+        e0.record()
+        tiny.fill_(i)
+        e1.record()
+        torch.cuda.synchronize()
+        empty.append(e0.elapsed_time(e1) * 1e-3)
+    del flush
+    cold_s = statistics.median(cold[2:])
+    line["dslash"]["cold_l2"] = {
+        "us_per_apply": 1e6 * cold_s, "GBps": dslash_bytes(V, R) / cold_s / 1e9,
+        "frac_of_peak": dslash_bytes(V, R) / cold_s / 1e9 / peak,
+        "bracket_us_around_a_trivial_kernel": 1e6 * statistics.median(empty[2:]),
+        "what": "one isolated launch after a 512 MB L2 flush, CUDA events around it (launch ramp and the "
+                "bracket's own cost included; the ncu kernel duration under the same conditions is in "
+                "profiles/r01_dslash_full_cfg3.md)"}
+
     if not args.no_solve:
         line["cg"] = {"s_per_solve": t_c_sum / K, "iterations": iters,
                       "us_per_iteration": 1e6 * (t_c_sum / K) / max(iters, 1), "nshift": cfg.nshift,
