@@ -21,7 +21,11 @@
  *                             (a full colour vector is 6 V doubles)
  *  Internal layout            the library's own parity-split, site-fastest SoA ("ap(V,3)",
  *              PAPER.md:210): an internal vector is 6*(V/2) doubles, opaque to the caller;
- *              qcd_pack / qcd_unpack convert.  All internal vectors must be 16-byte aligned.
+ *              qcd_pack / qcd_unpack convert.
+ *  Alignment   EVERY device buffer passed to the library (canonical links and vectors, internal
+ *              vectors, d_x, d_y) must be 16-byte aligned -- they are accessed with 16-byte loads
+ *              and stores -- and input and output ranges must not overlap; either violation
+ *              returns QCD_EINVAL before anything is launched.
  *  Pointers    d_* = DEVICE memory owned by the caller (e.g. torch.empty(...).data_ptr());
  *              h_* = HOST memory owned by the caller.  The library owns only its handle, its
  *              reordered gauge copy and its workspace, all released by qcd_destroy.
@@ -49,7 +53,8 @@ typedef struct qcd_ctx qcd_ctx; /* opaque; owned by the library */
 typedef enum {
     QCD_OK = 0,
     QCD_EINVAL = 1,   /* bad argument: odd or < 2 extent, NULL pointer, negative shift, nshift < 1 or
-                         > QCD_MAX_SHIFTS, tol <= 0, bad parity, aliasing in/out */
+                         > QCD_MAX_SHIFTS, tol <= 0, bad parity, overlapping in/out ranges, a device
+                         pointer that is not 16-byte aligned */
     QCD_ENOMEM = 2,   /* device or host allocation failed */
     QCD_ECUDA = 3,    /* CUDA error, or no sm_100 device */
     QCD_ENOTCONV = 4, /* max_iter reached; outputs are still written and true_res filled */
@@ -110,9 +115,17 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     conj(row_0 x row_1) (tolerance 1e-10 per component), SYNCHRONISES to read the
  *                     verdict and returns QCD_EINVAL (no field loaded) if a link fails.  Results differ
  *                     from the 3-row path at rounding level only (relative 1e-15).
+ *   QCD_OPT_DSLASH_KERNEL  which Dslash kernel every entry point uses.  0: links loaded straight into
+ *                     registers (thread per site, LDG.128).  1: links staged through shared memory by
+ *                     the bulk-copy engine (cp.async.bulk behind an mbarrier ring, a producer warp per
+ *                     CTA).  Bit-identical results.
+ *   QCD_OPT_DSLASH_PERSIST (default 0) with kernel 1: 0 launches one CTA per 128-site tile; n > 0
+ *                     launches a persistent grid of n CTAs per SM that walk the tiles round-robin.
+ *                     Dslash and M^dag M stay bit-identical; CG results change at rounding level only
+ *                     (the <p,Ap> partial sums are added per CTA).
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
-       QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6 };
+       QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */
@@ -146,6 +159,7 @@ QCD_API qcd_status qcd_mdagm(qcd_ctx *ctx, int parity, const double *d_in, doubl
  *   shifts     host, nshift values >= 0;   residues: host, nshift values (c_k of eq. 8)
  *   d_x        nshift internal vectors, contiguous, caller's shift order; may be NULL
  *   d_y        internal vector, y = sum_k residues[k] x_k (eq. 8 without c_0, C14); may be NULL
+ *              d_b, d_x and d_y must not overlap one another (QCD_EINVAL)
  *   iterations host int;  true_res: host, nshift doubles, ||b - (M^dag M + sigma_k) x_k|| / ||b||
  *              recomputed from x_k (not the recursion value).
  * Returns QCD_OK, or QCD_ENOTCONV if max_iter iterations did not reach tol. Synchronises. */
@@ -161,10 +175,12 @@ QCD_API qcd_status qcd_multishift_cg(qcd_ctx *ctx, int parity, const double *d_b
  * approximation of type (n, n) on [xmin, xmax] -- what the paper takes from Mathematica's MiniMax
  * (appendix :288-304), computed here from Zolotarev's closed form in double precision:
  *   c0       host, 1 double;   coef, shift: host, n doubles each (c_k > 0; d_k > 0, ascending)
- *   delta    host, may be NULL: max over [xmin, xmax] of |1 - sqrt(x) r(x)|
+ *   delta    host, may be NULL: max over [xmin, xmax] of |1 - sqrt(x) r(x)| (formed in double
+ *            precision from two function values: not resolved below ~1e-15)
  * The caller chooses xmin < lambda_min(M^dag M) (>= m^2 in this normalisation) and
  * xmax > lambda_max (m^2 + 4 for unit links, about 7 for random SU(3), never above m^2 + 16; the
- * paper keeps xmax = 34 in its normalisation, which is 8.5 here).  QCD_EINVAL unless 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax.
+ * paper keeps xmax = 34 in its normalisation, which is 8.5 here).  QCD_EINVAL unless
+ * 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax; QCD_ENOTCONV if a coefficient is not finite.
  *
  * qcd_inv_sqrt: d_out = c_0 d_phi + sum_k c_k (M^dag M + d_k)^(-1) d_phi on `parity` with those
  * coefficients, by ONE multishift CG (n shifts) and a fused combine.  Arguments as

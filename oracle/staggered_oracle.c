@@ -226,11 +226,6 @@ static double re_dot(long n, const cplx *a, const cplx *b)
     return (double)s;
 }
 
-double orc_norm2(long n_complex, const double *a)
-{
-    return re_dot(n_complex, (const cplx *)a, (const cplx *)a);
-}
-
 /* ||b - (A + sigma) x|| / ||b||, recomputed from scratch (not a recursion value) */
 static double true_residual(orc_lattice *L, double mass, int parity, double sigma,
                             const cplx *b, const cplx *x, cplx *work, cplx *rout)

@@ -16,7 +16,7 @@ import numpy as np
 
 QCD_EVEN, QCD_ODD = 0, 1
 QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH, QCD_OPT_LINK_ROWS, QCD_OPT_TGROUP = 0, 1, 2, 3, 4
-QCD_OPT_L2_PERSIST_MB, QCD_OPT_Y_ONLY = 5, 6
+QCD_OPT_L2_PERSIST_MB, QCD_OPT_Y_ONLY, QCD_OPT_DSLASH_KERNEL, QCD_OPT_DSLASH_PERSIST = 5, 6, 7, 8
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONV, QCD_ESTATE = range(6)
 _STATUS_NAMES = ["QCD_OK", "QCD_EINVAL", "QCD_ENOMEM", "QCD_ECUDA", "QCD_ENOTCONV", "QCD_ESTATE"]
 
@@ -104,16 +104,20 @@ for _n in _SIGNATURES:
     globals()[_n] = _make_raw(_n)
 
 
-def _dev_ptr(t) -> int:
-    """Address of a contiguous float64 CUDA tensor."""
+def _dev_ptr(t, doubles: int | None = None) -> int:
+    """Address of a contiguous float64 CUDA tensor (holding at least `doubles` elements)."""
     if not (t.is_cuda and t.is_contiguous() and str(t.dtype) == "torch.float64"):
         raise TypeError("expected a contiguous float64 CUDA tensor")
+    if doubles is not None and t.numel() < doubles:
+        raise ValueError(f"device buffer holds {t.numel()} doubles, the call needs {doubles}")
     return t.data_ptr()
 
 
-def _host_ptr(a: np.ndarray) -> int:
+def _host_ptr(a: np.ndarray, doubles: int | None = None) -> int:
     if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags.c_contiguous):
         raise TypeError("expected a C-contiguous float64 numpy array")
+    if doubles is not None and a.size < doubles:
+        raise ValueError(f"host buffer holds {a.size} doubles, the call needs {doubles}")
     return a.ctypes.data
 
 
@@ -191,22 +195,22 @@ class Context:
 
     # -- device entry points --
     def load_gauge(self, d_links):
-        self._check(self._lib.qcd_load_gauge(self._h, _dev_ptr(d_links)), "qcd_load_gauge")
+        self._check(self._lib.qcd_load_gauge(self._h, _dev_ptr(d_links, 72 * self.volume)), "qcd_load_gauge")
 
     def pack(self, parity: int, d_canonical, d_internal):
-        self._check(self._lib.qcd_pack(self._h, parity, _dev_ptr(d_canonical), _dev_ptr(d_internal)),
+        self._check(self._lib.qcd_pack(self._h, parity, _dev_ptr(d_canonical, self.vector_doubles), _dev_ptr(d_internal, self.vector_doubles)),
                     "qcd_pack")
 
     def unpack(self, parity: int, d_internal, d_canonical):
-        self._check(self._lib.qcd_unpack(self._h, parity, _dev_ptr(d_internal), _dev_ptr(d_canonical)),
+        self._check(self._lib.qcd_unpack(self._h, parity, _dev_ptr(d_internal, self.vector_doubles), _dev_ptr(d_canonical, self.vector_doubles)),
                     "qcd_unpack")
 
     def dslash(self, out_parity: int, d_in, d_out):
-        self._check(self._lib.qcd_dslash(self._h, out_parity, _dev_ptr(d_in), _dev_ptr(d_out)),
+        self._check(self._lib.qcd_dslash(self._h, out_parity, _dev_ptr(d_in, self.vector_doubles), _dev_ptr(d_out, self.vector_doubles)),
                     "qcd_dslash")
 
     def mdagm(self, parity: int, d_in, d_out):
-        self._check(self._lib.qcd_mdagm(self._h, parity, _dev_ptr(d_in), _dev_ptr(d_out)), "qcd_mdagm")
+        self._check(self._lib.qcd_mdagm(self._h, parity, _dev_ptr(d_in, self.vector_doubles), _dev_ptr(d_out, self.vector_doubles)), "qcd_mdagm")
 
     def multishift_cg(self, parity: int, d_b, shifts, residues, tol: float, max_iter: int,
                       d_x=None, d_y=None):
@@ -214,12 +218,14 @@ class Context:
         shifts = np.ascontiguousarray(shifts, dtype=np.float64)
         residues = np.ascontiguousarray(residues, dtype=np.float64)
         n = int(shifts.size)
+        if residues.size != n:
+            raise ValueError("shifts and residues must have the same length")
         true_res = np.full(n, np.nan)
         it = _ci(0)
         st = self._lib.qcd_multishift_cg(
-            self._h, parity, _dev_ptr(d_b), n, _host_ptr(shifts), _host_ptr(residues), float(tol),
-            int(max_iter), None if d_x is None else _dev_ptr(d_x),
-            None if d_y is None else _dev_ptr(d_y), ctypes.byref(it), _host_ptr(true_res))
+            self._h, parity, _dev_ptr(d_b, self.vector_doubles), n, _host_ptr(shifts), _host_ptr(residues), float(tol),
+            int(max_iter), None if d_x is None else _dev_ptr(d_x, n * self.vector_doubles),
+            None if d_y is None else _dev_ptr(d_y, self.vector_doubles), ctypes.byref(it), _host_ptr(true_res))
         self._check(st, "qcd_multishift_cg", allow=(QCD_ENOTCONV,))
         return st, it.value, true_res
 
@@ -229,8 +235,8 @@ class Context:
         true_res = np.full(int(n), np.nan)
         delta = np.zeros(1)
         it = _ci(0)
-        st = self._lib.qcd_inv_sqrt(self._h, parity, _dev_ptr(d_phi), int(n), float(xmin), float(xmax),
-                                    float(tol), int(max_iter), _dev_ptr(d_out), ctypes.byref(it),
+        st = self._lib.qcd_inv_sqrt(self._h, parity, _dev_ptr(d_phi, self.vector_doubles), int(n), float(xmin), float(xmax),
+                                    float(tol), int(max_iter), _dev_ptr(d_out, self.vector_doubles), ctypes.byref(it),
                                     _host_ptr(true_res), _host_ptr(delta))
         self._check(st, "qcd_inv_sqrt", allow=(QCD_ENOTCONV,))
         return st, it.value, true_res, float(delta[0])
@@ -241,23 +247,23 @@ class Context:
         true_res = np.full(int(n), np.nan)
         delta = np.zeros(1)
         it = _ci(0)
-        st = self._lib.qcd_apply_pow(self._h, parity, _dev_ptr(d_phi), int(num), int(den), int(n),
+        st = self._lib.qcd_apply_pow(self._h, parity, _dev_ptr(d_phi, self.vector_doubles), int(num), int(den), int(n),
                                      float(xmin), float(xmax), float(tol), int(max_iter),
-                                     _dev_ptr(d_out), ctypes.byref(it), _host_ptr(true_res),
+                                     _dev_ptr(d_out, self.vector_doubles), ctypes.byref(it), _host_ptr(true_res),
                                      _host_ptr(delta))
         self._check(st, "qcd_apply_pow", allow=(QCD_ENOTCONV,))
         return st, it.value, true_res, float(delta[0])
 
     # -- host entry points (canonical numpy arrays; copies happen inside the C call) --
     def load_gauge_host(self, h_links: np.ndarray):
-        self._check(self._lib.qcd_load_gauge_host(self._h, _host_ptr(h_links)), "qcd_load_gauge_host")
+        self._check(self._lib.qcd_load_gauge_host(self._h, _host_ptr(h_links, 72 * self.volume)), "qcd_load_gauge_host")
 
     def dslash_host(self, out_parity: int, h_in: np.ndarray, h_out: np.ndarray):
-        self._check(self._lib.qcd_dslash_host(self._h, out_parity, _host_ptr(h_in), _host_ptr(h_out)),
+        self._check(self._lib.qcd_dslash_host(self._h, out_parity, _host_ptr(h_in, self.vector_doubles), _host_ptr(h_out, self.vector_doubles)),
                     "qcd_dslash_host")
 
     def mdagm_host(self, parity: int, h_in: np.ndarray, h_out: np.ndarray):
-        self._check(self._lib.qcd_mdagm_host(self._h, parity, _host_ptr(h_in), _host_ptr(h_out)),
+        self._check(self._lib.qcd_mdagm_host(self._h, parity, _host_ptr(h_in, self.vector_doubles), _host_ptr(h_out, self.vector_doubles)),
                     "qcd_mdagm_host")
 
     def multishift_cg_host(self, parity: int, h_b: np.ndarray, shifts, residues, tol: float,
@@ -266,11 +272,13 @@ class Context:
         shifts = np.ascontiguousarray(shifts, dtype=np.float64)
         residues = np.ascontiguousarray(residues, dtype=np.float64)
         n = int(shifts.size)
+        if residues.size != n:
+            raise ValueError("shifts and residues must have the same length")
         true_res = np.full(n, np.nan)
         it = _ci(0)
         st = self._lib.qcd_multishift_cg_host(
-            self._h, parity, _host_ptr(h_b), n, _host_ptr(shifts), _host_ptr(residues), float(tol),
-            int(max_iter), None if h_x is None else _host_ptr(h_x),
-            None if h_y is None else _host_ptr(h_y), ctypes.byref(it), _host_ptr(true_res))
+            self._h, parity, _host_ptr(h_b, self.vector_doubles), n, _host_ptr(shifts), _host_ptr(residues), float(tol),
+            int(max_iter), None if h_x is None else _host_ptr(h_x, n * self.vector_doubles),
+            None if h_y is None else _host_ptr(h_y, self.vector_doubles), ctypes.byref(it), _host_ptr(true_res))
         self._check(st, "qcd_multishift_cg_host", allow=(QCD_ENOTCONV,))
         return st, it.value, true_res

@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdint>
 #include <cstring>
 #include <new>
 #include <string>
@@ -55,14 +56,16 @@ struct qcd_ctx {
     unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
     bool opt_y_only = false;            // qcd_inv_sqrt / qcd_apply_pow accumulate y directly, no x_k
     int opt_cg_batch = 8;               // iterations enqueued per batch / per graph
+    int opt_dslash_kernel = 0;          // 0: register-staged links (dslash.cu); 1: bulk-copy staged (dslash_bulk.cu)
+    int opt_dslash_persist = 0;         // bulk kernel: CTAs per SM of a persistent grid (0: one CTA per tile)
     // cached graph of one batch of CG iterations (valid for exactly the key below)
     cudaGraphExec_t cg_exec = nullptr;
     cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
     struct CgKey {
-        int parity = -1, batch = 0, rows = 0; bool pdl = false, apw = false, yonly = false; double mass = 0.0;
+        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0; bool pdl = false, apw = false, yonly = false; double mass = 0.0;
         const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
         bool operator==(const CgKey &o) const {
-            return parity == o.parity && batch == o.batch && rows == o.rows && pdl == o.pdl && apw == o.apw && yonly == o.yonly && mass == o.mass &&
+            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && pdl == o.pdl && apw == o.apw && yonly == o.yonly && mass == o.mass &&
                    x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
         }
     } cg_key;
@@ -137,6 +140,15 @@ void setup_l2_window(qcd_ctx *c)
 
 bool bad_parity(int p) { return p != QCD_EVEN && p != QCD_ODD; }
 
+// every device buffer is accessed with 16-byte loads and stores (double2)
+bool misaligned(const void *p) { return ((uintptr_t)p & 15u) != 0; }
+// [a, a + na) and [b, b + nb) (bytes) share at least one byte
+bool overlap(const void *a, size_t na, const void *b, size_t nb)
+{
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    return x < y + nb && y < x + na;
+}
+
 qcd_status ensure_host_staging(qcd_ctx *c)
 {
     if (!c->stage_vec) QCD_CUDA(c, cudaMalloc((void **)&c->stage_vec, c->vec_bytes));
@@ -175,7 +187,8 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->partial;
     p.st = (gated || dot_mode || coeff_from_state) ? c->st : nullptr;
-    c->launches += launch_dslash(c->g, p, c->Ld());
+    if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(c->g, p, c->opt_dslash_persist, c->Ld());
+    else c->launches += launch_dslash(c->g, p, c->Ld());
     return QCD_OK;
 }
 
@@ -197,7 +210,7 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
 qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y_only)
 {
     qcd_ctx::CgKey key;
-    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
+    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.kern = c->opt_dslash_kernel; key.persist = c->opt_dslash_persist; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
     key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp;
     if (c->cg_exec && key == c->cg_key) return QCD_OK;
     if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }
@@ -378,6 +391,14 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }   // Geom is baked in
         return QCD_OK;
     case QCD_OPT_Y_ONLY: c->opt_y_only = value != 0; return QCD_OK;
+    case QCD_OPT_DSLASH_KERNEL:
+        if (value != 0 && value != 1) return fail(c, QCD_EINVAL, "qcd_set_option: Dslash kernel must be 0 or 1");
+        c->opt_dslash_kernel = (int)value;
+        return QCD_OK;
+    case QCD_OPT_DSLASH_PERSIST:
+        if (value < 0 || value > 8) return fail(c, QCD_EINVAL, "qcd_set_option: CTAs per SM must be in [0, 8]");
+        c->opt_dslash_persist = (int)value;
+        return QCD_OK;
     case QCD_OPT_L2_PERSIST_MB:
         if (value < 0) return fail(c, QCD_EINVAL, "qcd_set_option: L2 persist size must be >= 0");
         c->opt_l2_persist_mb = value;
@@ -397,7 +418,8 @@ const char *qcd_last_error(const qcd_ctx *c) { return c ? c->err.c_str() : g_cre
 qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
 {
     if (!c) return QCD_EINVAL;
-    if (!d_links) return fail(c, QCD_EINVAL, "qcd_load_gauge: NULL links");
+    if (!d_links || misaligned(d_links))
+        return fail(c, QCD_EINVAL, "qcd_load_gauge: NULL or misaligned (16 bytes) links");
     int *flag = &c->st->not_su3;
     QCD_CUDA(c, cudaMemsetAsync(flag, 0, sizeof(int), c->stream));
     c->gauge_loaded = false;
@@ -432,8 +454,9 @@ qcd_status qcd_load_gauge_host(qcd_ctx *c, const double *h_links)
 qcd_status qcd_pack(qcd_ctx *c, int parity, const double *d_canon, double *d_internal)
 {
     if (!c) return QCD_EINVAL;
-    if (bad_parity(parity) || !d_canon || !d_internal || d_canon == d_internal)
-        return fail(c, QCD_EINVAL, "qcd_pack: bad argument");
+    if (bad_parity(parity) || !d_canon || !d_internal || misaligned(d_canon) || misaligned(d_internal) ||
+        overlap(d_canon, c->vec_bytes, d_internal, c->vec_bytes))
+        return fail(c, QCD_EINVAL, "qcd_pack: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
     c->launches += launch_pack(c->g, d_canon, (double2 *)d_internal, c->L());
     return check_launch(c, "qcd_pack");
 }
@@ -441,8 +464,9 @@ qcd_status qcd_pack(qcd_ctx *c, int parity, const double *d_canon, double *d_int
 qcd_status qcd_unpack(qcd_ctx *c, int parity, const double *d_internal, double *d_canon)
 {
     if (!c) return QCD_EINVAL;
-    if (bad_parity(parity) || !d_canon || !d_internal || d_canon == d_internal)
-        return fail(c, QCD_EINVAL, "qcd_unpack: bad argument");
+    if (bad_parity(parity) || !d_canon || !d_internal || misaligned(d_canon) || misaligned(d_internal) ||
+        overlap(d_canon, c->vec_bytes, d_internal, c->vec_bytes))
+        return fail(c, QCD_EINVAL, "qcd_unpack: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
     c->launches += launch_unpack(c->g, (const double2 *)d_internal, d_canon, c->L());
     return check_launch(c, "qcd_unpack");
 }
@@ -450,8 +474,9 @@ qcd_status qcd_unpack(qcd_ctx *c, int parity, const double *d_internal, double *
 qcd_status qcd_dslash(qcd_ctx *c, int out_parity, const double *d_in, double *d_out)
 {
     if (!c) return QCD_EINVAL;
-    if (bad_parity(out_parity) || !d_in || !d_out || d_in == d_out)
-        return fail(c, QCD_EINVAL, "qcd_dslash: bad argument");
+    if (bad_parity(out_parity) || !d_in || !d_out || misaligned(d_in) || misaligned(d_out) ||
+        overlap(d_in, c->vec_bytes, d_out, c->vec_bytes))
+        return fail(c, QCD_EINVAL, "qcd_dslash: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_dslash: no gauge field loaded");
     run_dslash(c, out_parity, (const double2 *)d_in, (double2 *)d_out, nullptr, 0.0, false, 0, false);
     return check_launch(c, "qcd_dslash");
@@ -460,8 +485,9 @@ qcd_status qcd_dslash(qcd_ctx *c, int out_parity, const double *d_in, double *d_
 qcd_status qcd_mdagm(qcd_ctx *c, int parity, const double *d_in, double *d_out)
 {
     if (!c) return QCD_EINVAL;
-    if (bad_parity(parity) || !d_in || !d_out || d_in == d_out)
-        return fail(c, QCD_EINVAL, "qcd_mdagm: bad argument");
+    if (bad_parity(parity) || !d_in || !d_out || misaligned(d_in) || misaligned(d_out) ||
+        overlap(d_in, c->vec_bytes, d_out, c->vec_bytes))
+        return fail(c, QCD_EINVAL, "qcd_mdagm: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_mdagm: no gauge field loaded");
     const double2 *in = (const double2 *)d_in;
     run_dslash(c, 1 - parity, in, c->tmp, nullptr, 0.0, false, 0, false);
@@ -488,6 +514,13 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         return fail(c, QCD_EINVAL, "qcd_multishift_cg: tol must be > 0 and max_iter >= 1");
     for (int k = 0; k < nshift; ++k)
         if (!(shifts[k] >= 0.0)) return fail(c, QCD_EINVAL, "qcd_multishift_cg: shifts must be >= 0");
+    if (misaligned(d_b) || misaligned(d_x) || misaligned(d_y))
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg: device buffers must be 16-byte aligned");
+    // x is zeroed before b is read and y is written while b and x are read: no overlap allowed
+    if ((d_x && overlap(d_b, c->vec_bytes, d_x, c->vec_bytes * nshift)) ||
+        (d_y && overlap(d_b, c->vec_bytes, d_y, c->vec_bytes)) ||
+        (d_x && d_y && overlap(d_y, c->vec_bytes, d_x, c->vec_bytes * nshift)))
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg: d_b, d_x and d_y must not overlap");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_multishift_cg: no gauge field loaded");
     y_only = y_only && d_x == nullptr && d_y != nullptr;
     qcd_status s = ensure_cg_workspace(c, nshift, d_x == nullptr && !y_only);
@@ -578,11 +611,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         c->launches += launch_dslash_multi(c->g, mp, c->Ld());
     }
     if (y_only) {
-        if (with_c0) {      // y <- c0 b + 1 * y, in place (every thread reads its element before writing it)
-            const long long zero = 0;
-            const double one = 1.0;
-            c->launches += launch_combine(n2, x, &zero, &one, 1, c0, b, x, c->L());
-        }
+        if (with_c0) c->launches += launch_add_c0(n2, c0, b, x, c->L());      // y += c0 b, in place
     } else if (d_y)
         c->launches += launch_combine(n2, x, xoff_caller.data(), residues, nshift, c0,
                                       with_c0 ? b : nullptr, (double2 *)d_y, c->L());
@@ -624,7 +653,11 @@ qcd_status qcd_inv_sqrt_coeffs(int n, double xmin, double xmax, double *c0, doub
 {
     if (!c0 || !coef || !shift)
         return fail(nullptr, QCD_EINVAL, "qcd_inv_sqrt_coeffs: NULL output");
-    if (zolotarev_inv_sqrt(n, xmin, xmax, c0, coef, shift, delta) != 0)
+    const int rc = zolotarev_inv_sqrt(n, xmin, xmax, c0, coef, shift, delta);
+    if (rc == 2)
+        return fail(nullptr, QCD_ENOTCONV, "qcd_inv_sqrt_coeffs: a coefficient is not representable in "
+                                           "double precision for this n and interval");
+    if (rc != 0)
         return fail(nullptr, QCD_EINVAL,
                     "qcd_inv_sqrt_coeffs: need 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax");
     return QCD_OK;
@@ -649,7 +682,8 @@ qcd_status qcd_apply_pow(qcd_ctx *c, int parity, const double *d_phi, int num, i
                          int *iterations, double *true_res, double *delta)
 {
     if (!c) return QCD_EINVAL;
-    if (!d_out || d_out == d_phi) return fail(c, QCD_EINVAL, "qcd_apply_pow: bad output pointer");
+    if (!d_out || !d_phi || overlap(d_phi, c->vec_bytes, d_out, c->vec_bytes))
+        return fail(c, QCD_EINVAL, "qcd_apply_pow: NULL or overlapping d_phi / d_out");
     const qcd_ctx::PowFit *fit = nullptr;
     for (const auto &f : c->pow_cache)
         if (f.num == num && f.den == den && f.n == n && f.xmin == xmin && f.xmax == xmax) fit = &f;
@@ -672,10 +706,11 @@ qcd_status qcd_inv_sqrt(qcd_ctx *c, int parity, const double *d_phi, int n, doub
                         double *true_res, double *delta)
 {
     if (!c) return QCD_EINVAL;
-    if (!d_out || d_out == d_phi) return fail(c, QCD_EINVAL, "qcd_inv_sqrt: bad output pointer");
+    if (!d_out || !d_phi || overlap(d_phi, c->vec_bytes, d_out, c->vec_bytes))
+        return fail(c, QCD_EINVAL, "qcd_inv_sqrt: NULL or overlapping d_phi / d_out");
     double c0, coef[kMaxShifts], shift[kMaxShifts];
-    if (zolotarev_inv_sqrt(n, xmin, xmax, &c0, coef, shift, delta) != 0)
-        return fail(c, QCD_EINVAL, "qcd_inv_sqrt: need 1 <= n <= QCD_MAX_SHIFTS and 0 < xmin < xmax");
+    const qcd_status cs = qcd_inv_sqrt_coeffs(n, xmin, xmax, &c0, coef, shift, delta);
+    if (cs != QCD_OK) return fail(c, cs, qcd_last_error(nullptr));
     return multishift_cg_impl(c, parity, d_phi, n, shift, coef, tol, max_iter, nullptr, d_out,
                               iterations, true_res, true, c0, c->opt_y_only);
 }

@@ -215,6 +215,22 @@ combine_kernel(long n2, const double2 *__restrict__ x, const CombineArgs a, doub
     }
 }
 
+// y += c_0 b, in place: the c_0 term of eq. 8 on the y-only path, where y has been accumulated by the
+// iteration itself (a kernel of its own: y is read and written through the same, unrestricted pointer)
+__global__ void __launch_bounds__(kBlock)
+add_c0_kernel(long n2, double c0, const double2 *__restrict__ b, double2 *y)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        const double2 v = __ldg(b + i);
+        double2 s = y[i];
+        s.x = fma(c0, v.x, s.x);
+        s.y = fma(c0, v.y, s.y);
+        y[i] = s;
+    }
+}
+
 }  // namespace
 
 int blas_grid_blocks(long n2)
@@ -258,6 +274,12 @@ int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p,
     long blocks = (n2 + kBlock - 1) / kBlock;
     int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
     launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, r, y, p, pstride, st);
+    return 1;
+}
+
+int launch_add_c0(long n2, double c0, const double2 *b, double2 *y, Launch L)
+{
+    launch_kernel(add_c0_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, c0, b, y);
     return 1;
 }
 

@@ -70,17 +70,24 @@ struct Site {
 // showed 2.7-2.8 GB of DRAM reads per apply against 2.52 GB algorithmic), while each group still
 // streams tgroup * 2 KB contiguous bytes of every link plane.  tgroup == chunks: plain h order.
 // SIGNS: also derive eta_mu(x) and the t-seam signs (needed when the links are stored without them).
-template <bool SIGNS>
-__device__ __forceinline__ void locate(const Geom &g, int par, Site &s)
+// tile (= CTA of the one-tile-per-CTA kernels) -> t-slice and first site of its chunk inside the slice
+__device__ __forceinline__ void tile_origin(const Geom &g, uint32_t tile, uint32_t &t, uint32_t &sl0)
 {
     const uint32_t per_group = (uint32_t)g.tgroup * (uint32_t)g.nt_run;
-    const uint32_t grp = blockIdx.x / per_group, rem = blockIdx.x - grp * per_group;
+    const uint32_t grp = tile / per_group, rem = tile - grp * per_group;
     const uint32_t first = grp * (uint32_t)g.tgroup;
     const uint32_t width = min((uint32_t)g.tgroup, (uint32_t)g.chunks - first);   // chunks in this group
     const uint32_t tq = rem / width;
-    const uint32_t t = (uint32_t)g.t0 + tq;
-    const uint32_t chunk = first + (rem - tq * width);
-    const uint32_t sl = chunk * kDslashBlock + threadIdx.x;    // index inside the t-slice
+    t = (uint32_t)g.t0 + tq;
+    sl0 = (first + (rem - tq * width)) * kDslashBlock;
+}
+
+template <bool SIGNS>
+__device__ __forceinline__ void locate_tile(const Geom &g, int par, uint32_t tile, uint32_t lane, Site &s)
+{
+    uint32_t t, sl0;
+    tile_origin(g, tile, t, sl0);
+    const uint32_t sl = sl0 + lane;    // index inside the t-slice
     s.valid = sl < (uint32_t)g.st;
     const uint32_t h = t * (uint32_t)g.st + sl;
     s.h = h;
@@ -115,6 +122,12 @@ __device__ __forceinline__ void locate(const Geom &g, int par, Site &s)
             s.nb[3] = e3 ^ (t == 0);                     // s- on the hop t = 0 -> Nt-1
         }
     }
+}
+
+template <bool SIGNS>
+__device__ __forceinline__ void locate(const Geom &g, int par, Site &s)
+{
+    locate_tile<SIGNS>(g, par, blockIdx.x, threadIdx.x, s);
 }
 
 // u[0 .. 3*ROWS) <- the stored entries of one link (plane stride Vh); ROWS == 2: rebuild row 2.

@@ -148,6 +148,9 @@ struct DslashParams {
     CgState *st;               // also the early-exit flag when non-null
 };
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L);
+// dslash_bulk.cu: the same operator with the links staged through shared memory by cp.async.bulk;
+// ctas_per_sm > 0: persistent grid of that many CTAs per SM, 0: one CTA per 128-site tile
+int launch_dslash_bulk(const Geom &g, const DslashParams &p, int ctas_per_sm, Launch L);
 int dslash_grid_blocks(const Geom &g);
 int dslash_chunks(const Geom &g);
 
@@ -188,6 +191,9 @@ int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, l
 // y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
                    int nshift, double c0, const double2 *b, double2 *y, Launch L);
+
+// y += c0 b in place (the c_0 term of eq. 8 on the y-only path)
+int launch_add_c0(long n2, double c0, const double2 *b, double2 *y, Launch L);
 
 // host only (zolotarev.cu): minimax x^(-1/2) ~= c0 + sum_k c[k]/(x + d[k]) on [xmin, xmax]; 0 = ok
 int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, double *d, double *delta);

@@ -85,7 +85,7 @@ int zolotarev_data(int n, double xmin, double xmax, double *a, double *ref)
     return 0;
 }
 
-// Returns 0, or 1 for bad arguments.  c and d hold n doubles each, d ascending.
+// Returns 0, 1 for bad arguments, 2 if a coefficient is not finite.  c and d hold n doubles each, d ascending.
 int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, double *d, double *delta)
 {
     double a[2 * kMaxShifts + 2], ref[2 * kMaxShifts + 2];
@@ -104,13 +104,18 @@ int zolotarev_inv_sqrt(int n, double xmin, double xmax, double *c0, double *c, d
     *c0 = D / s;
     for (int k = 1; k <= n; ++k) {
         const double dk = a[2 * k - 1];
-        double v = D;
-        for (int l = 1; l <= n; ++l) v *= a[2 * l] - dk;
-        for (int j = 1; j <= n; ++j)
-            if (j != k) v /= a[2 * j - 1] - dk;
+        // numerator and denominator factors taken in pairs: the interlacing a_1 < a_2 < ... keeps every
+        // ratio and every partial product bounded (by xmax/xmin), where the product of all n numerator
+        // factors alone grows like (xmax/xmin)^(n/2) and overflows for large n on wide intervals
+        double v = D * (a[2 * k] - dk);
+        for (int l = 1; l <= n; ++l)
+            if (l != k) v *= (a[2 * l] - dk) / (a[2 * l - 1] - dk);
         c[k - 1] = v * s;
         d[k - 1] = dk * xmin;
     }
+    if (!std::isfinite(*c0)) return 2;
+    for (int k = 0; k < n; ++k)
+        if (!std::isfinite(c[k]) || !std::isfinite(d[k]) || !(d[k] > 0.0)) return 2;
     return 0;
 }
 

@@ -42,6 +42,18 @@ def test_library_coefficients_meet_their_own_delta(n, xmin, xmax):
     assert np.abs(err).max() >= 0.999 * delta
 
 
+def test_wide_interval_with_the_maximum_number_of_poles_stays_finite():
+    """The product of the n numerator factors of a residue grows like (xmax/xmin)^(n/2): 1e448 for
+    n = 64 on [1e-12, 100].  The library pairs numerator and denominator factors, so every coefficient
+    stays finite and agrees with the 50-digit oracle."""
+    n, xmin, xmax = 64, 1e-12, 100.0
+    c0, c, d, delta = q.inv_sqrt_coeffs(n, xmin, xmax)
+    z = R.zolotarev_inv_sqrt(n, xmin, xmax)
+    assert np.isfinite(c).all() and np.isfinite(d).all() and np.isfinite(c0)
+    assert abs(c0 / z["c0"] - 1) <= 1e-8
+    assert np.abs(c / z["c"] - 1).max() <= 1e-8 and np.abs(d / z["d"] - 1).max() <= 1e-8
+
+
 def test_bad_arguments():
     lib = q.load_library()
     buf = (ctypes.c_double * 8)()
@@ -87,6 +99,33 @@ def test_pow_library_meets_its_own_delta_and_the_papers_figure():
     assert np.abs(err).max() >= 0.99 * delta
     # 'about 30 coefficients to achieve an error below 1e-11' at xmin < (2 m a)^2 = 1.6e-5
     assert q.pow_coeffs(1, 4, 30, 1.6e-5, 34.0)[3] < 1e-11
+
+
+def _extrema(err):
+    """indices of the local extrema of |err| (end points included)"""
+    a = np.abs(err)
+    idx = [i for i in range(len(a))
+           if (i == 0 or a[i] >= a[i - 1]) and (i == len(a) - 1 or a[i] > a[i + 1])]
+    return [i for i in idx if a[i] > 0.5 * a.max()]
+
+
+@pytest.mark.parametrize("num,den,n,xmin,xmax", [(1, 4, 10, 2.5e-5, 8.5), (-1, 3, 7, 1e-3, 8.5),
+                                                  (-1, 2, 8, 1e-4, 8.5), (1, 4, 6, 1e-3, 7.0)])
+def test_library_fits_satisfy_chebyshevs_criterion(num, den, n, xmin, xmax):
+    """Independent of the oracle's Remez (which uses the same algorithm as csrc/remez.cu): a type-(n,n)
+    rational function whose relative error reaches +-delta with alternating sign at 2n+2 points of
+    [xmin, xmax], end points included, IS the minimax approximation (it is unique).  The LIBRARY's
+    coefficients are evaluated in 50 digits (evaluation only) and checked for exactly that: the count,
+    the alternation, the level, the end points."""
+    c0, c, d, delta = q.pow_coeffs(num, den, n, xmin, xmax)
+    x = xmin * (xmax / xmin) ** (np.arange(6001) / 6000.0)
+    err = R.relative_error_curve_pow(num / den, c0, c, d, x)
+    ext = _extrema(err)
+    assert len(ext) == 2 * n + 2 and ext[0] == 0 and ext[-1] == len(x) - 1
+    signs = np.sign(err[ext])
+    assert (signs[1:] * signs[:-1] < 0).all()
+    assert np.abs(np.abs(err[ext]) / delta - 1).max() < 2e-4
+    assert abs(np.abs(err).max() / delta - 1) < 1e-6
 
 
 def test_pow_minus_one_half_is_the_closed_form():
