@@ -31,7 +31,8 @@ struct qcd_ctx {
     double2 *tmp = nullptr, *q = nullptr, *r = nullptr;
     double2 *p = nullptr;  int p_cap = 0;
     double2 *xws = nullptr; int x_cap = 0;
-    double *partial = nullptr;
+    double *partial = nullptr;          // per-CTA partial sums of the ticketed reductions
+    double *pap_partial = nullptr;      // per-CTA partial sums of <p_0,q>, written by the Dslash, read by the r-update
     CgState *st = nullptr;
     double *results = nullptr;          // device, kMaxShifts doubles
     CgState *h_state = nullptr;         // pinned
@@ -185,7 +186,7 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     p.W = c->W; p.link_rows = c->link_rows; p.in = in; p.out = out; p.out_parity = out_parity;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
-    p.dot_mode = dot_mode; p.partial = c->partial;
+    p.dot_mode = dot_mode; p.partial = c->pap_partial;
     p.st = (gated || dot_mode || coeff_from_state) ? c->st : nullptr;
     if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(c->g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(c->g, p, c->Ld());
@@ -198,7 +199,9 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
     // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
     run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
     run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
-    c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->partial, c->st, c->loop_handle, c->L());
+    const int npap = c->opt_dslash_kernel == 1 ? dslash_bulk_grid_blocks(c->g, c->opt_dslash_persist)
+                                               : dslash_grid_blocks(c->g);
+    c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, c->st, c->loop_handle, c->L());
     if (y_only)      // `x` is the single vector y
         c->launches += launch_cg_update_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
     else
@@ -320,6 +323,7 @@ qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx
     if (dev_alloc(&c->W, (size_t)72 * g.Vh) != cudaSuccess ||
         dev_alloc(&c->tmp, (size_t)c->n2) != cudaSuccess ||
         dev_alloc(&c->partial, (size_t)nblk * kMultiRhs) != cudaSuccess ||
+        dev_alloc(&c->pap_partial, (size_t)dslash_grid_blocks(g)) != cudaSuccess ||
         dev_alloc(&c->st, 1) != cudaSuccess ||
         dev_alloc(&c->results, (size_t)kMaxShifts + 1) != cudaSuccess)
         return cleanup(QCD_ENOMEM, "qcd_create: device allocation failed");
@@ -342,7 +346,7 @@ qcd_status qcd_destroy(qcd_ctx *c)
     if (c->cg_exec) cudaGraphExecDestroy(c->cg_exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaFree(c->W); cudaFree(c->tmp); cudaFree(c->q); cudaFree(c->r); cudaFree(c->p);
-    cudaFree(c->xws); cudaFree(c->partial); cudaFree(c->st); cudaFree(c->results);
+    cudaFree(c->xws); cudaFree(c->partial); cudaFree(c->pap_partial); cudaFree(c->st); cudaFree(c->results);
     if (c->s_in) cudaStreamDestroy(c->s_in);
     if (c->s_out) cudaStreamDestroy(c->s_out);
     for (auto &e : c->ev_pipe) if (e) cudaEventDestroy(e);

@@ -38,14 +38,24 @@ cg_init_kernel(long n2, const double2 *__restrict__ b, double2 *__restrict__ r,
     }
 }
 
-// r -= alpha q ; rho' = <r,r> ; last block: beta, beta_k, zeta rotation, freezing, stop test
+// r -= alpha q ; rho' = <r,r> ; last block: zeta_new, alpha_k, beta, beta_k, zeta rotation, freezing,
+// stop test.  alpha = rho / <p_0,q> is formed here, by every CTA for itself, from the per-CTA partial
+// sums the second Dslash of the iteration left in pap_partial[0 .. npap): same loads, same order, same
+// tree in every CTA, so all CTAs hold the same bits (and runs repeat bit for bit).  That takes the
+// ticket, the fence and the serial last-block pass out of the stencil: one reduction tail per
+// iteration instead of two.
 // LOOP: the kernel is a node of the WHILE graph of QCD_OPT_CG_GRAPH = 2 and sets its condition.  A
 // separate instantiation, because a kernel that references the device-side graph API is invisible to
 // ncu (the launch list of the default path would lose its r-update rows).
+constexpr int kRUnroll = 4;                       // independent 16-byte loads per array per thread
+constexpr int kRChunk = kBlock * kRUnroll;
+constexpr int kRMaxBlocks = 148 * 4;
+
 template <bool LOOP>
 __global__ void __launch_bounds__(kBlock)
-cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q, double *partial,
-                   CgState *st, cudaGraphConditionalHandle loop)
+cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q,
+                   const double *__restrict__ pap_partial, int npap, double *partial, CgState *st,
+                   cudaGraphConditionalHandle loop)
 {
     pdl_wait();
     pdl_launch_dependents();
@@ -56,18 +66,33 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
         }
         return;
     }
-    const double alpha = st->alpha;
+    double t = 0.0;
+    for (int i = threadIdx.x; i < npap; i += kBlock) t += __ldcg(pap_partial + i);
+    const double pAp = block_sum<kBlock>(t);
+    const double alpha = st->rho / pAp;   // st->rho is rewritten by the last block only, after every CTA has read it
     double s = 0.0;
-    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
-        double2 rv = r[i];
-        const double2 qv = __ldg(q + i);
-        rv.x = fma(-alpha, qv.x, rv.x);
-        rv.y = fma(-alpha, qv.y, rv.y);
-        r[i] = rv;
-        s += rv.x * rv.x + rv.y * rv.y;
+    for (long base = (long)blockIdx.x * kRChunk + threadIdx.x; base < n2; base += (long)gridDim.x * kRChunk) {
+        double2 rv[kRUnroll], qv[kRUnroll];
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) { rv[e] = r[i]; qv[e] = __ldg(q + i); }
+        }
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) {
+                rv[e].x = fma(-alpha, qv[e].x, rv[e].x);
+                rv[e].y = fma(-alpha, qv[e].y, rv[e].y);
+                r[i] = rv[e];
+                s += rv[e].x * rv[e].x + rv[e].y * rv[e].y;
+            }
+        }
     }
     double total;
     if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total)) {
+        cg_step_alpha(st, pAp);
+        __syncthreads();
         cg_step_beta(st, total);
         // device-side loop (QCD_OPT_CG_GRAPH = 2): this iteration's shift update still runs (it is part
         // of the loop body); the WHILE node then stops when the stop test above has set `done`
@@ -246,14 +271,21 @@ int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstri
     return 1;
 }
 
-int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
-                       unsigned long long loop_handle, Launch L)
+int cg_update_r_grid_blocks(long n2)
 {
+    long b = (n2 + kRChunk - 1) / kRChunk;
+    return (int)(b < kRMaxBlocks ? (b > 0 ? b : 1) : kRMaxBlocks);
+}
+
+int launch_cg_update_r(long n2, double2 *r, const double2 *q, const double *pap_partial, int npap,
+                       double *partial, CgState *st, unsigned long long loop_handle, Launch L)
+{
+    const int grid = cg_update_r_grid_blocks(n2);
     if (loop_handle)
-        launch_kernel(cg_update_r_kernel<true>, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st,
+        launch_kernel(cg_update_r_kernel<true>, grid, kBlock, L.s, L.pdl, n2, r, q, pap_partial, npap, partial, st,
                       (cudaGraphConditionalHandle)loop_handle);
     else
-        launch_kernel(cg_update_r_kernel<false>, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, r, q, partial, st,
+        launch_kernel(cg_update_r_kernel<false>, grid, kBlock, L.s, L.pdl, n2, r, q, pap_partial, npap, partial, st,
                       (cudaGraphConditionalHandle)0);
     return 1;
 }

@@ -1,8 +1,8 @@
 // dslash.cu -- a2/a3/a4 of SURVEY 8(a): the even-odd staggered Dirac operator
 //   out(x) = sum_mu [ W_mu(x) in(x+mu) - W_mu(x-mu)^dag in(x-mu) ],  x of parity out_parity
 // (PAPER.md:106 with 1/2, eta and the t-seam sign folded into W, see layout.cu), optionally fused
-// with out = coeff*src - (.) (the m^2 term of M^dag M) and with the partial sums of
-// Re<src,out> whose last block runs the CG alpha/zeta step.
+// with out = coeff*src - (.) (the m^2 term of M^dag M) and with per-CTA partial sums
+// of Re<src,out>, from which the CG's r-update forms alpha.
 //
 // HBM-bound stencil: 8 links (1152 B) + 48 B out per site, neighbour vectors mostly from L2/L1;
 // 570 flop / 1248 B = 0.46 flop/B, so no tensor cores (BASELINE.json north_star).  One thread per
@@ -134,9 +134,10 @@ dslash_kernel(const Geom g, const DslashParams p)
         for (int c = 0; c < 3; ++c) p.out[(long)c * Vh + h] = acc[c];
     }
     if (DOT) {
-        double total;
-        if (grid_sum_last_block<kBlock>(dot, p.partial, &p.st->counter, total))
-            cg_step_alpha(p.st, total);
+        // one partial sum per CTA; the r-update, which needs alpha, adds them up itself (blas.cu): no
+        // ticket, no fence and no serial last-block pass at the end of the stencil
+        const double b = block_sum<kBlock>(dot);
+        if (threadIdx.x == 0) p.partial[blockIdx.x] = b;
     }
 }
 

@@ -271,10 +271,9 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
             }
         }
     }
-    if (DOT) {
-        double total;
-        if (grid_sum_last_block<kThreads>(dot, p.partial, &p.st->counter, total))
-            cg_step_alpha(p.st, total);
+    if (DOT) {      // one partial per CTA, summed by the r-update (blas.cu)
+        const double b = block_sum<kThreads>(dot);
+        if (threadIdx.x == 0) p.partial[blockIdx.x] = b;
     }
 }
 
@@ -310,11 +309,16 @@ cudaError_t launch_one(const Geom &g, const DslashParams &p, int grid, uint32_t 
 
 // persistent != 0: at most persistent CTAs per SM x 148 SMs walk the tiles round-robin (the producer
 // streams across tile boundaries); 0: one CTA per tile
+int dslash_bulk_grid_blocks(const Geom &g, int ctas_per_sm)
+{
+    const int ntiles = dslash_grid_blocks(g);
+    return ctas_per_sm > 0 ? std::min(ntiles, 148 * ctas_per_sm) : ntiles;
+}
+
 int launch_dslash_bulk(const Geom &g, const DslashParams &p, int ctas_per_sm, Launch L)
 {
     const int ntiles = dslash_grid_blocks(g);
-    int grid = ntiles;
-    if (ctas_per_sm > 0) grid = std::min(ntiles, 148 * ctas_per_sm);
+    const int grid = dslash_bulk_grid_blocks(g, ctas_per_sm);
     const uint32_t nt = (uint32_t)ntiles;
     if (p.link_rows == 2) {
         if (p.src == nullptr) launch_one<false, false, 2>(g, p, grid, nt, L);

@@ -105,8 +105,11 @@ dslash_multi_kernel(const Geom g, const DslashMultiParams p)
     if (RES) {
         double total[NR];
         if (grid_sum_last_block_n<kBlock, NR>(sum, p.partial, p.counter, total)) {
-            if (threadIdx.x == 0)
-                for (int j = 0; j < p.nrhs; ++j) *p.result[j] = total[j];
+            if (threadIdx.x == 0) {
+#pragma unroll
+                for (int j = 0; j < NR; ++j)       // unrolled: `total` stays in registers (no stack frame)
+                    if (j < p.nrhs) *p.result[j] = total[j];
+            }
         }
     }
 }

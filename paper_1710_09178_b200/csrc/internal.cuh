@@ -142,8 +142,8 @@ struct DslashParams {
     double coeff;              // used when coeff_from_state == 0
     int coeff_from_state;      // 1: coeff = mass2 + st->sigma0 read on device
     double mass2;
-    // optional fused <src,out> with the CG alpha/zeta step in the last block
-    int dot_mode;              // 0 none, 1 CG (pAp -> alpha, zeta_new, coef_a)
+    // optional fused <src,out>: one partial sum per CTA in partial[blockIdx] (the CG's r-update adds them)
+    int dot_mode;              // 0 none, 1 on
     double *partial;
     CgState *st;               // also the early-exit flag when non-null
 };
@@ -151,6 +151,7 @@ int launch_dslash(const Geom &g, const DslashParams &p, Launch L);
 // dslash_bulk.cu: the same operator with the links staged through shared memory by cp.async.bulk;
 // ctas_per_sm > 0: persistent grid of that many CTAs per SM, 0: one CTA per 128-site tile
 int launch_dslash_bulk(const Geom &g, const DslashParams &p, int ctas_per_sm, Launch L);
+int dslash_bulk_grid_blocks(const Geom &g, int ctas_per_sm);
 int dslash_grid_blocks(const Geom &g);
 int dslash_chunks(const Geom &g);
 
@@ -181,8 +182,9 @@ int blas_grid_blocks(long n2);
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
                    double *partial, CgState *st, Launch L);
 // loop_handle != 0: the kernel is a node of a WHILE conditional graph and sets its condition
-int launch_cg_update_r(long n2, double2 *r, const double2 *q, double *partial, CgState *st,
-                       unsigned long long loop_handle, Launch L);
+// pap_partial[0 .. npap): the per-CTA partial sums of <p_0,q> the preceding Dslash wrote
+int launch_cg_update_r(long n2, double2 *r, const double2 *q, const double *pap_partial, int npap,
+                       double *partial, CgState *st, unsigned long long loop_handle, Launch L);
 // y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept)
 int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p, long pstride,
                               CgState *st, Launch L);
