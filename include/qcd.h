@@ -123,9 +123,23 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     launches a persistent grid of n CTAs per SM that walk the tiles round-robin.
  *                     Dslash and M^dag M stay bit-identical; CG results change at rounding level only
  *                     (the <p,Ap> partial sums are added per CTA).
+ *   QCD_OPT_MIXED     (default 0) SURVEY 8(f) NEXT-3, the mixed-precision variant the paper sets aside
+ *                     (PAPER.md:168).  With 1, the NEXT qcd_load_gauge also stores an fp32 copy of the
+ *                     three-row links (+288 V bytes), and qcd_multishift_cg becomes: (1) the fp64
+ *                     multishift CG down to 10^-QCD_OPT_MIXED_SWITCH_EXP only; (2) every shift on its
+ *                     own by defect correction -- residual with the fp64 operator, inner single-shift CG
+ *                     on the fp32-link operator (fp64 arithmetic and vectors, half the link bytes),
+ *                     x_k += e -- until the recomputed fp64 residual is <= tol.  Same results within
+ *                     the same tolerances; `iterations` counts stage 1 plus all inner iterations.
+ *                     qcd_inv_sqrt / qcd_apply_pow keep the fp64 solver.
+ *   QCD_OPT_MIXED_SWITCH_EXP (default 5) the loose tolerance of stage 1 is 10^-value, 1 <= value <= 15.
+ *   QCD_OPT_OPERATOR_LINKS32 (default 0) with 1, qcd_dslash and qcd_mdagm apply the operator built on
+ *                     the fp32 copy of the links (QCD_ESTATE unless the field was loaded with
+ *                     QCD_OPT_MIXED = 1): the inner operator of the mixed solver on its own.
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
-       QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8 };
+       QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8,
+       QCD_OPT_MIXED = 9, QCD_OPT_MIXED_SWITCH_EXP = 10, QCD_OPT_OPERATOR_LINKS32 = 11 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */
@@ -146,6 +160,15 @@ QCD_API qcd_status qcd_unpack(qcd_ctx *ctx, int parity, const double *d_internal
  * out_parity = QCD_ODD is D_oe (even in, odd out), QCD_EVEN is D_eo.  Internal layout; d_in and
  * d_out must not alias. */
 QCD_API qcd_status qcd_dslash(qcd_ctx *ctx, int out_parity, const double *d_in, double *d_out);
+
+/* The same stencil restricted to the t-slices t0 <= t < t0 + nt of the output (all other sites of d_out are
+ * left untouched), optionally fused with d_out = coeff * d_src - (D d_in) (d_src on out_parity, may be NULL).
+ * This is the building block of a t-slab decomposition (PAPER.md:146-148 slices along z; SURVEY 8(f)
+ * NEXT-4): a rank holds its slab plus one halo slice on either side as a lattice of its own and computes
+ * the interior slices only (paper_1710_09178_b200/slab.py).  QCD_EINVAL unless 0 <= t0, nt >= 1,
+ * t0 + nt <= Nt.  Does not synchronise. */
+QCD_API qcd_status qcd_dslash_range(qcd_ctx *ctx, int out_parity, const double *d_in, double *d_out,
+                                    int t0, int nt, const double *d_src, double coeff);
 
 /* a4: d_out = m^2 d_in - D_{p,q} D_{q,p} d_in on `parity` p  (C3).
  * Internal layout; d_in and d_out must not alias. */

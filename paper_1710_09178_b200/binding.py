@@ -17,6 +17,7 @@ import numpy as np
 QCD_EVEN, QCD_ODD = 0, 1
 QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH, QCD_OPT_LINK_ROWS, QCD_OPT_TGROUP = 0, 1, 2, 3, 4
 QCD_OPT_L2_PERSIST_MB, QCD_OPT_Y_ONLY, QCD_OPT_DSLASH_KERNEL, QCD_OPT_DSLASH_PERSIST = 5, 6, 7, 8
+QCD_OPT_MIXED, QCD_OPT_MIXED_SWITCH_EXP, QCD_OPT_OPERATOR_LINKS32 = 9, 10, 11
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONV, QCD_ESTATE = range(6)
 _STATUS_NAMES = ["QCD_OK", "QCD_EINVAL", "QCD_ENOMEM", "QCD_ECUDA", "QCD_ENOTCONV", "QCD_ESTATE"]
 
@@ -38,6 +39,7 @@ _SIGNATURES = {
     "qcd_pack": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_unpack": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_dslash": (_ci, [_vp, _ci, _vp, _vp]),
+    "qcd_dslash_range": (_ci, [_vp, _ci, _vp, _vp, _ci, _ci, _vp, _cd]),
     "qcd_mdagm": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_multishift_cg": (_ci, [_vp, _ci, _vp, _ci, _vp, _vp, _cd, _ci, _vp, _vp,
                                 ctypes.POINTER(_ci), _vp]),
@@ -208,6 +210,12 @@ class Context:
     def dslash(self, out_parity: int, d_in, d_out):
         self._check(self._lib.qcd_dslash(self._h, out_parity, _dev_ptr(d_in, self.vector_doubles), _dev_ptr(d_out, self.vector_doubles)),
                     "qcd_dslash")
+
+    def dslash_range(self, out_parity: int, d_in, d_out, t0: int, nt: int, d_src=None, coeff: float = 0.0):
+        vd = self.vector_doubles
+        self._check(self._lib.qcd_dslash_range(self._h, out_parity, _dev_ptr(d_in, vd), _dev_ptr(d_out, vd),
+                                               int(t0), int(nt), None if d_src is None else _dev_ptr(d_src, vd),
+                                               float(coeff)), "qcd_dslash_range")
 
     def mdagm(self, parity: int, d_in, d_out):
         self._check(self._lib.qcd_mdagm(self._h, parity, _dev_ptr(d_in, self.vector_doubles), _dev_ptr(d_out, self.vector_doubles)), "qcd_mdagm")

@@ -57,19 +57,29 @@ struct qcd_ctx {
     unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
     bool opt_y_only = false;            // qcd_inv_sqrt / qcd_apply_pow accumulate y directly, no x_k
     int opt_cg_batch = 8;               // iterations enqueued per batch / per graph
+    // NEXT-3 (mixed precision): fp32 copy of the three-row links and the buffers of the refinement
+    float2 *W32 = nullptr;
+    bool links32_loaded = false;
+    bool opt_mixed = false;             // QCD_OPT_MIXED: build W32 at the next load; qcd_multishift_cg refines per shift
+    int opt_mixed_switch_exp = 5;       // stage 1 stops at 10^-exp
+    bool opt_operator_links32 = false;  // qcd_dslash / qcd_mdagm apply the fp32-link operator
+    bool use_links32 = false;           // transient: the launches being enqueued use W32
+    double2 *mx_r = nullptr, *mx_e = nullptr;
     int opt_dslash_kernel = 0;          // 0: register-staged links (dslash.cu); 1: bulk-copy staged (dslash_bulk.cu)
     int opt_dslash_persist = 0;         // bulk kernel: CTAs per SM of a persistent grid (0: one CTA per tile)
     // cached graph of one batch of CG iterations (valid for exactly the key below)
-    cudaGraphExec_t cg_exec = nullptr;
+    cudaGraphExec_t cg_exec = nullptr;  // the entry of cg_cache selected by the last ensure_cg_graph
     cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
     struct CgKey {
-        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0; bool pdl = false, apw = false, yonly = false; double mass = 0.0;
+        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0; bool pdl = false, apw = false, yonly = false, l32 = false; double mass = 0.0;
         const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
         bool operator==(const CgKey &o) const {
-            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && pdl == o.pdl && apw == o.apw && yonly == o.yonly && mass == o.mass &&
+            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && pdl == o.pdl && apw == o.apw && yonly == o.yonly && l32 == o.l32 && mass == o.mass &&
                    x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
         }
-    } cg_key;
+    };
+    struct CgGraph { CgKey key; cudaGraphExec_t exec; };
+    std::vector<CgGraph> cg_cache;      // a few graphs: the mixed-precision solve alternates between two
     // L2 persistence of part of the gauge field (set at qcd_load_gauge; apw_on == false: none)
     cudaAccessPolicyWindow apw{};
     bool apw_on = false;
@@ -184,11 +194,12 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
 {
     DslashParams p{};
     p.W = c->W; p.link_rows = c->link_rows; p.in = in; p.out = out; p.out_parity = out_parity;
+    p.W32 = c->W32; p.links32 = c->use_links32 ? 1 : 0;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->pap_partial;
     p.st = (gated || dot_mode || coeff_from_state) ? c->st : nullptr;
-    if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(c->g, p, c->opt_dslash_persist, c->Ld());
+    if (c->opt_dslash_kernel == 1 && !c->use_links32) c->launches += launch_dslash_bulk(c->g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(c->g, p, c->Ld());
     return QCD_OK;
 }
@@ -199,7 +210,7 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
     // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
     run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
     run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
-    const int npap = c->opt_dslash_kernel == 1 ? dslash_bulk_grid_blocks(c->g, c->opt_dslash_persist)
+    const int npap = c->opt_dslash_kernel == 1 && !c->use_links32 ? dslash_bulk_grid_blocks(c->g, c->opt_dslash_persist)
                                                : dslash_grid_blocks(c->g);
     c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, c->st, c->loop_handle, c->L());
     if (y_only)      // `x` is the single vector y
@@ -214,9 +225,11 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y
 {
     qcd_ctx::CgKey key;
     key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.kern = c->opt_dslash_kernel; key.persist = c->opt_dslash_persist; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
-    key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp;
-    if (c->cg_exec && key == c->cg_key) return QCD_OK;
-    if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }
+    key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp; key.l32 = c->use_links32;
+    for (auto &e : c->cg_cache)
+        if (e.key == key) { c->cg_exec = e.exec; return QCD_OK; }
+    c->cg_exec = nullptr;
+    if (c->cg_cache.size() >= 4) { cudaGraphExecDestroy(c->cg_cache.front().exec); c->cg_cache.erase(c->cg_cache.begin()); }
     if (!c->cap_stream)
         QCD_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
     cudaStream_t user = c->stream;
@@ -267,7 +280,7 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y
         c->cg_exec = nullptr;
         return fail(c, QCD_ECUDA, std::string("CG graph capture: ") + cudaGetErrorString(e));
     }
-    c->cg_key = key;
+    c->cg_cache.push_back({key, c->cg_exec});
     return QCD_OK;
 }
 
@@ -343,7 +356,7 @@ qcd_status qcd_destroy(qcd_ctx *c)
 {
     if (!c) return QCD_OK;
     cudaStreamSynchronize(c->stream);
-    if (c->cg_exec) cudaGraphExecDestroy(c->cg_exec);
+    for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     cudaFree(c->W); cudaFree(c->tmp); cudaFree(c->q); cudaFree(c->r); cudaFree(c->p);
     cudaFree(c->xws); cudaFree(c->partial); cudaFree(c->pap_partial); cudaFree(c->st); cudaFree(c->results);
@@ -352,7 +365,7 @@ qcd_status qcd_destroy(qcd_ctx *c)
     for (auto &e : c->ev_pipe) if (e) cudaEventDestroy(e);
     cudaFree(c->stage_out);
     cudaFree(c->stage_links); cudaFree(c->stage_vec); cudaFree(c->hv_a); cudaFree(c->hv_b);
-    cudaFree(c->hv_y);
+    cudaFree(c->hv_y); cudaFree(c->W32); cudaFree(c->mx_r); cudaFree(c->mx_e);
     if (c->h_state) cudaFreeHost(c->h_state);
     if (c->h_done) cudaFreeHost(c->h_done);
     if (c->h_results) cudaFreeHost(c->h_results);
@@ -392,9 +405,16 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
     case QCD_OPT_TGROUP:
         if (value < 0) return fail(c, QCD_EINVAL, "qcd_set_option: tgroup must be >= 0");
         c->g.tgroup = value == 0 ? auto_tgroup(c->g) : value > c->g.chunks ? c->g.chunks : (int)value;
-        if (c->cg_exec) { cudaGraphExecDestroy(c->cg_exec); c->cg_exec = nullptr; }   // Geom is baked in
+        for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);   // Geom is baked in
+        c->cg_cache.clear(); c->cg_exec = nullptr;
         return QCD_OK;
     case QCD_OPT_Y_ONLY: c->opt_y_only = value != 0; return QCD_OK;
+    case QCD_OPT_MIXED: c->opt_mixed = value != 0; return QCD_OK;
+    case QCD_OPT_MIXED_SWITCH_EXP:
+        if (value < 1 || value > 15) return fail(c, QCD_EINVAL, "qcd_set_option: switch exponent must be in [1, 15]");
+        c->opt_mixed_switch_exp = (int)value;
+        return QCD_OK;
+    case QCD_OPT_OPERATOR_LINKS32: c->opt_operator_links32 = value != 0; return QCD_OK;
     case QCD_OPT_DSLASH_KERNEL:
         if (value != 0 && value != 1) return fail(c, QCD_EINVAL, "qcd_set_option: Dslash kernel must be 0 or 1");
         c->opt_dslash_kernel = (int)value;
@@ -436,6 +456,13 @@ qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
         if (c->h_done[0])
             return fail(c, QCD_EINVAL, "qcd_load_gauge: two-row storage needs links in SU(3); a third row "
                                        "differs from conj(row0 x row1) by more than 1e-10");
+    }
+    c->links32_loaded = false;
+    if (c->opt_mixed) {                 // NEXT-3: fp32 copy of the (three-row) links for the inner operator
+        if (!c->W32) QCD_CUDA(c, dev_alloc(&c->W32, (size_t)72 * c->g.Vh));
+        c->launches += launch_ingest_links32(c->g, d_links, c->W32, c->L());
+        if ((s = check_launch(c, "qcd_load_gauge (fp32 copy)")) != QCD_OK) return s;
+        c->links32_loaded = true;
     }
     c->gauge_loaded = true; c->link_rows = c->opt_link_rows; setup_l2_window(c);
     c->fresh_gauge = true;
@@ -482,8 +509,32 @@ qcd_status qcd_dslash(qcd_ctx *c, int out_parity, const double *d_in, double *d_
         overlap(d_in, c->vec_bytes, d_out, c->vec_bytes))
         return fail(c, QCD_EINVAL, "qcd_dslash: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_dslash: no gauge field loaded");
+    if (c->opt_operator_links32 && !c->links32_loaded)
+        return fail(c, QCD_ESTATE, "qcd_dslash: QCD_OPT_OPERATOR_LINKS32 needs a gauge field loaded with QCD_OPT_MIXED = 1");
+    c->use_links32 = c->opt_operator_links32;
     run_dslash(c, out_parity, (const double2 *)d_in, (double2 *)d_out, nullptr, 0.0, false, 0, false);
+    c->use_links32 = false;
     return check_launch(c, "qcd_dslash");
+}
+
+qcd_status qcd_dslash_range(qcd_ctx *c, int out_parity, const double *d_in, double *d_out, int t0, int nt,
+                            const double *d_src, double coeff)
+{
+    if (!c) return QCD_EINVAL;
+    if (bad_parity(out_parity) || !d_in || !d_out || misaligned(d_in) || misaligned(d_out) || misaligned(d_src) ||
+        overlap(d_in, c->vec_bytes, d_out, c->vec_bytes) || (d_src && overlap(d_src, c->vec_bytes, d_out, c->vec_bytes)))
+        return fail(c, QCD_EINVAL, "qcd_dslash_range: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
+    if (t0 < 0 || nt < 1 || t0 + nt > c->g.Nt)
+        return fail(c, QCD_EINVAL, "qcd_dslash_range: need 0 <= t0, 1 <= nt, t0 + nt <= Nt");
+    if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_dslash_range: no gauge field loaded");
+    Geom g = c->g;
+    g.t0 = t0; g.nt_run = nt;
+    DslashParams p{};
+    p.W = c->W; p.link_rows = c->link_rows; p.in = (const double2 *)d_in; p.out = (double2 *)d_out;
+    p.out_parity = out_parity; p.src = (const double2 *)d_src; p.coeff = coeff;
+    if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(g, p, c->opt_dslash_persist, c->Ld());
+    else c->launches += launch_dslash(g, p, c->Ld());
+    return check_launch(c, "qcd_dslash_range");
 }
 
 qcd_status qcd_mdagm(qcd_ctx *c, int parity, const double *d_in, double *d_out)
@@ -493,9 +544,13 @@ qcd_status qcd_mdagm(qcd_ctx *c, int parity, const double *d_in, double *d_out)
         overlap(d_in, c->vec_bytes, d_out, c->vec_bytes))
         return fail(c, QCD_EINVAL, "qcd_mdagm: bad parity, NULL, misaligned (16 bytes) or overlapping buffers");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_mdagm: no gauge field loaded");
+    if (c->opt_operator_links32 && !c->links32_loaded)
+        return fail(c, QCD_ESTATE, "qcd_mdagm: QCD_OPT_OPERATOR_LINKS32 needs a gauge field loaded with QCD_OPT_MIXED = 1");
     const double2 *in = (const double2 *)d_in;
+    c->use_links32 = c->opt_operator_links32;
     run_dslash(c, 1 - parity, in, c->tmp, nullptr, 0.0, false, 0, false);
     run_dslash(c, parity, c->tmp, (double2 *)d_out, in, c->mass * c->mass, false, 0, false);
+    c->use_links32 = false;
     return check_launch(c, "qcd_mdagm");
 }
 
@@ -507,7 +562,8 @@ namespace {
 qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nshift,
                               const double *shifts, const double *residues, double tol,
                               int max_iter, double *d_x, double *d_y, int *iterations,
-                              double *true_res, bool with_c0, double c0, bool y_only = false)
+                              double *true_res, bool with_c0, double c0, bool y_only = false,
+                              bool finish = true)
 {
     if (!c) return QCD_EINVAL;
     if (bad_parity(parity) || !d_b || !shifts || !residues || !iterations || !true_res)
@@ -595,7 +651,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
 
     // finish (a6): true residuals recomputed from x_k, kMultiRhs shifts per pass over the links;
     // the p_k are dead by now and serve as the tmp vectors.  y = sum_k c_k x_k.
-    for (int k0 = 0; k0 < (y_only ? 0 : nshift); k0 += kMultiRhs) {
+    for (int k0 = 0; k0 < (y_only || !finish ? 0 : nshift); k0 += kMultiRhs) {
         const int nb = std::min(kMultiRhs, nshift - k0);
         DslashMultiParams mp{};
         mp.W = c->W; mp.link_rows = c->link_rows; mp.nrhs = nb;
@@ -630,12 +686,82 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     const double rho_b = h.rho_b;
     for (int k = 0; k < nshift; ++k)
         true_res[k] = rho_b > 0.0 ? std::sqrt(c->h_results[k] / rho_b) : 0.0;
-    if (y_only)      // no x_k to recompute from: the recursion's own estimate |zeta_k| sqrt(rho/rho_b),
+    if (y_only || !finish)      // no x_k to recompute from: the recursion's own estimate |zeta_k| sqrt(rho/rho_b),
         for (int k = 0; k < nshift; ++k)        // and the freezing threshold for the frozen shifts
             true_res[order[k]] = rho_b > 0.0 ? (h.active[k] ? std::fabs(h.zeta[k]) * std::sqrt(h.rho / rho_b)
                                                             : h.freeze * tol) : 0.0;
     const bool converged = rho_b == 0.0 || std::sqrt(h.rho / rho_b) <= tol;
     if (!converged) return fail(c, QCD_ENOTCONV, "qcd_multishift_cg: max_iter reached");
+    return QCD_OK;
+}
+
+// SURVEY 8(f) NEXT-3 (reading N3; oracle/mixed_precision.py): the mixed-precision
+// form of the solve.  Stage 1: the fp64 multishift CG down to the loose tolerance 10^-switch_exp.
+// Stage 2: every shift on its own by defect correction -- outer residual with the fp64 operator, inner
+// single-shift CG on the fp32-link operator (dslash_kernel<.,.,3,float2>) to
+// tau = max(tol ||b|| / (2 ||r||), 1e-2), x_k += e -- until ||b - (A + sigma_k) x_k|| <= tol ||b||.
+// `iterations` = stage-1 iterations + all inner iterations.
+qcd_status mixed_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshift, const double *shifts,
+                               const double *residues, double tol, int max_iter, double *d_x, double *d_y,
+                               int *iterations, double *true_res)
+{
+    constexpr int kMaxRounds = 60;
+    constexpr double kInnerFloor = 1e-2;
+    if (!iterations || !true_res) return fail(c, QCD_EINVAL, "qcd_multishift_cg: NULL argument");
+    const double loose = std::max(tol, std::pow(10.0, -(double)c->opt_mixed_switch_exp));
+    qcd_status s = multishift_cg_impl(c, parity, d_b, nshift, shifts, residues, loose, max_iter, d_x, nullptr,
+                                      iterations, true_res, false, 0.0, false, /*finish=*/false);
+    if (s != QCD_OK && s != QCD_ENOTCONV) return s;
+    const long n2 = c->n2;
+    if (!c->mx_r) QCD_CUDA(c, dev_alloc(&c->mx_r, (size_t)n2));
+    if (!c->mx_e) QCD_CUDA(c, dev_alloc(&c->mx_e, (size_t)n2));
+    const double rho_b = c->h_state->rho_b;
+    std::vector<int> order(nshift);
+    for (int k = 0; k < nshift; ++k) order[k] = k;
+    std::stable_sort(order.begin(), order.end(), [&](int a, int bb) { return shifts[a] < shifts[bb]; });
+    std::vector<long long> xoff(nshift);                  // caller index -> offset of x_k
+    for (int k = 0; k < nshift; ++k) xoff[order[k]] = (long long)(d_x ? order[k] : k) * n2;
+    double2 *xbase = d_x ? (double2 *)d_x : c->xws;
+    const double2 *b = (const double2 *)d_b;
+    int total_it = *iterations;
+    bool all_ok = true;
+    for (int k = 0; k < nshift && rho_b > 0.0; ++k) {
+        double2 *xk = xbase + xoff[k];
+        const double coeff = c->mass * c->mass + shifts[k];
+        for (int round = 0;; ++round) {
+            // r = b - ((m^2 + sigma_k) x_k - D_{p,q} D_{q,p} x_k), fp64 links
+            run_dslash(c, 1 - parity, xk, c->tmp, nullptr, 0.0, false, 0, false);
+            run_dslash(c, parity, c->tmp, c->q, xk, coeff, false, 0, false);
+            c->launches += launch_residual(n2, b, c->q, c->mx_r, c->partial, &c->st->counter, c->results, c->L());
+            if ((s = check_launch(c, "qcd_multishift_cg (mixed)")) != QCD_OK) return s;
+            QCD_CUDA(c, cudaMemcpyAsync(c->h_results, c->results, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+            QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+            const double rr = c->h_results[0];
+            true_res[k] = std::sqrt(rr / rho_b);
+            if (true_res[k] <= tol) break;
+            if (round == kMaxRounds || total_it >= max_iter) { all_ok = false; break; }
+            const double tau = std::max(0.5 * tol / true_res[k], kInnerFloor);
+            const double one = 1.0;
+            int its = 0;
+            double tr_in = 0.0;
+            c->use_links32 = true;
+            s = multishift_cg_impl(c, parity, (const double *)c->mx_r, 1, &shifts[k], &one, tau,
+                                   std::max(1, max_iter - total_it), (double *)c->mx_e, nullptr, &its, &tr_in,
+                                   false, 0.0, false, /*finish=*/false);
+            c->use_links32 = false;
+            if (s != QCD_OK && s != QCD_ENOTCONV) return s;
+            total_it += its;
+            c->launches += launch_add_c0(n2, 1.0, c->mx_e, xk, c->L());     // x_k += e
+        }
+    }
+    if (rho_b == 0.0)
+        for (int k = 0; k < nshift; ++k) true_res[k] = 0.0;
+    if (d_y)
+        c->launches += launch_combine(n2, xbase, xoff.data(), residues, nshift, 0.0, nullptr, (double2 *)d_y, c->L());
+    if ((s = check_launch(c, "qcd_multishift_cg (mixed)")) != QCD_OK) return s;
+    QCD_CUDA(c, cudaStreamSynchronize(c->stream));
+    *iterations = total_it;
+    if (!all_ok) return fail(c, QCD_ENOTCONV, "qcd_multishift_cg (mixed): max_iter or the round limit reached");
     return QCD_OK;
 }
 
@@ -648,6 +774,9 @@ qcd_status qcd_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int nshi
                              int max_iter, double *d_x, double *d_y, int *iterations,
                              double *true_res)
 {
+    if (c && c->opt_mixed && c->links32_loaded)
+        return mixed_multishift_cg(c, parity, d_b, nshift, shifts, residues, tol, max_iter, d_x, d_y,
+                                   iterations, true_res);
     return multishift_cg_impl(c, parity, d_b, nshift, shifts, residues, tol, max_iter, d_x, d_y,
                               iterations, true_res, false, 0.0);
 }

@@ -256,6 +256,25 @@ add_c0_kernel(long n2, double c0, const double2 *__restrict__ b, double2 *y)
     }
 }
 
+// out = b - q ; *result = ||out||^2   (outer residual of the mixed-precision refinement, NEXT-3)
+__global__ void __launch_bounds__(kBlock)
+residual_kernel(long n2, const double2 *__restrict__ b, const double2 *__restrict__ q, double2 *__restrict__ out,
+                double *partial, unsigned *counter, double *result)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    double s = 0.0;
+    for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
+        const double2 bv = __ldg(b + i), qv = __ldg(q + i);
+        const double2 d = make_double2(bv.x - qv.x, bv.y - qv.y);
+        out[i] = d;
+        s += d.x * d.x + d.y * d.y;
+    }
+    double total;
+    if (grid_sum_last_block<kBlock>(s, partial, counter, total))
+        if (threadIdx.x == 0) *result = total;
+}
+
 }  // namespace
 
 int blas_grid_blocks(long n2)
@@ -306,6 +325,13 @@ int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p,
     long blocks = (n2 + kBlock - 1) / kBlock;
     int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
     launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, r, y, p, pstride, st);
+    return 1;
+}
+
+int launch_residual(long n2, const double2 *b, const double2 *q, double2 *out, double *partial, unsigned *counter,
+                    double *result, Launch L)
+{
+    launch_kernel(residual_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, q, out, partial, counter, result);
     return 1;
 }
 

@@ -33,12 +33,16 @@ constexpr int kBlock = kDslashBlock;
 // ROWS == 2: W holds rows 0 and 1 of the plain U; eta_mu(x), the t-seam sign and the 1/2 are applied
 //            here.  All of them depend on the OUTPUT site only: eta_mu does not depend on x_mu, and
 //            the seam sign of the backward hop is s-_mu(x).
-template <bool XPAY, bool DOT, int ROWS>
+// WT = double2: the links as stored (p.W).  WT = float2: the fp32 copy p.W32 (NEXT-3, inner operator of
+// the mixed-precision solver, three rows only); every entry is widened on load, the arithmetic is fp64.
+template <bool XPAY, bool DOT, int ROWS, class WT = double2>
 __global__ void __launch_bounds__(kBlock, ROWS == 2 ? QCD_DSLASH2_MINB : QCD_DSLASH3_MINB)
 dslash_kernel(const Geom g, const DslashParams p)
 {
     constexpr int NW = 3 * ROWS;
     const int Vh = g.Vh;
+    const WT *__restrict__ const W = sizeof(WT) == sizeof(float2) ? reinterpret_cast<const WT *>(p.W32)
+                                                                 : reinterpret_cast<const WT *>(p.W);
     Site site;
     locate<ROWS == 2>(g, p.out_parity, site);
     const bool valid = site.valid;
@@ -55,8 +59,8 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
         for (int k = 0; k < NPF; ++k) {
             const int mu = k >> 1;
-            if (k & 1) load_link<ROWS>(p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
-            else load_link<ROWS>(p.W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
+            if (k & 1) load_link<ROWS>(W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
+            else load_link<ROWS>(W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
         }
     };
     // Inside the CG, `done` was last written two or more kernels back (r-update), which has completed
@@ -76,7 +80,7 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
         for (int mu = 0; mu < 4; ++mu) {
             {   // forward hop: + W_mu(x) in(x+mu), link based at x (parity par)
-                const double2 *__restrict__ w = p.W + ((long)(par * 4 + mu) * NW) * Vh + h;
+                const WT *__restrict__ w = W + ((long)(par * 4 + mu) * NW) * Vh + h;
                 double2 u[9], v[3];
                 if (2 * mu < NPF) {
 #pragma unroll
@@ -96,7 +100,7 @@ dslash_kernel(const Geom g, const DslashParams p)
                     for (int b = 0; b < 3; ++b) cmad(acc[a], u[a * 3 + b], v[b]);
             }
             {   // backward hop: - W_mu(x-mu)^dag in(x-mu), link based at x-mu (parity 1-par)
-                const double2 *__restrict__ w = p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu];
+                const WT *__restrict__ w = W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu];
                 double2 u[9], v[3];
                 if (2 * mu + 1 < NPF) {
 #pragma unroll
@@ -149,7 +153,14 @@ int dslash_grid_blocks(const Geom &g) { return dslash_chunks(g) * g.nt_run; }
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
 {
     const int blocks = dslash_grid_blocks(g);
-    if (p.link_rows == 2) {
+    if (p.links32) {
+        if (p.src == nullptr)
+            launch_kernel_apw(dslash_kernel<false, false, 3, float2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        else if (p.dot_mode == 0)
+            launch_kernel_apw(dslash_kernel<true, false, 3, float2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        else
+            launch_kernel_apw(dslash_kernel<true, true, 3, float2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+    } else if (p.link_rows == 2) {
         if (p.src == nullptr)
             launch_kernel_apw(dslash_kernel<false, false, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
         else if (p.dot_mode == 0)

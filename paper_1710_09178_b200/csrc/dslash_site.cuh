@@ -130,11 +130,14 @@ __device__ __forceinline__ void locate(const Geom &g, int par, Site &s)
     locate_tile<SIGNS>(g, par, blockIdx.x, threadIdx.x, s);
 }
 
+__device__ __forceinline__ double2 widen(double2 v) { return v; }
+__device__ __forceinline__ double2 widen(float2 v) { return make_double2((double)v.x, (double)v.y); }
+
 // u[0 .. 3*ROWS) <- the stored entries of one link (plane stride Vh); ROWS == 2: rebuild row 2.
-template <int ROWS>
-__device__ __forceinline__ void load_link(const double2 *__restrict__ w, int Vh, double2 *u)
+// WT = double2, or float2 for the fp32 copy of the links (NEXT-3: the arithmetic stays fp64).
+template <int ROWS, class WT>
+__device__ __forceinline__ void load_link(const WT *__restrict__ w, int Vh, double2 *u)
 {
-#pragma unroll
     // Links are used exactly once per apply: load them with the streaming (evict-first) policy, so that
     // L2 keeps the vectors (the output of one Dslash is the gathered input of the next) and does not
     // cycle the whole gauge field through LRU.  Measured, us per apply at 32^3x8 / 48^3x12 / 64^3x16:
@@ -142,7 +145,8 @@ __device__ __forceinline__ void load_link(const double2 *__restrict__ w, int Vh,
 #ifndef QCD_LINK_LOAD
 #define QCD_LINK_LOAD __ldcs
 #endif
-    for (int i = 0; i < 3 * ROWS; ++i) u[i] = QCD_LINK_LOAD(w + (long)i * Vh);
+#pragma unroll
+    for (int i = 0; i < 3 * ROWS; ++i) u[i] = widen(QCD_LINK_LOAD(w + (long)i * Vh));
     if (ROWS == 2) third_row(u);
 }
 

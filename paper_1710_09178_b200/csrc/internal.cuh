@@ -127,12 +127,19 @@ struct Launch {
 // not_su3 (device int, zeroed by the caller): set to 1 by the two-row ingest when a link is not in SU(3)
 int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, int link_rows, int *not_su3,
                         Launch L);
+// fp32 copy of the three-row internal links: W32[2][4][9][Vh] = (float) 1/2 eta s+ U  (NEXT-3)
+int launch_ingest_links32(const Geom &g, const double *links_canon, float2 *W32, Launch L);
+// out = b - q, *result = ||out||^2 (one ticketed reduction)
+int launch_residual(long n2, const double2 *b, const double2 *q, double2 *out, double *partial, unsigned *counter,
+                    double *result, Launch L);
 // sites h0 <= h < h1 only (h1 < 0: all)
 int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L, int h0 = 0, int h1 = -1);
 int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L, int h0 = 0, int h1 = -1);
 
 struct DslashParams {
     const double2 *W;
+    const float2 *W32;         // fp32 copy of the three-row links (same layout), used when links32 != 0
+    int links32;
     int link_rows;             // 3: W[2][4][9][Vh] with signs folded in; 2: W[2][4][6][Vh] plain rows 0,1
     const double2 *in;
     double2 *out;

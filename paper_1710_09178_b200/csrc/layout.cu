@@ -63,6 +63,39 @@ ingest_links_kernel(Geom g, const double2 *__restrict__ U, double2 *__restrict__
     }
 }
 
+// fp32 copy of the three-row links (NEXT-3): the same W_mu(x) = 1/2 eta s+ U, every entry rounded to
+// fp32.  The factor is a signed power of two, so rounding commutes with it: W32 = 1/2 eta s+ fl32(U).
+__global__ void __launch_bounds__(kBlock)
+ingest_links32_kernel(Geom g, const double2 *__restrict__ U, float2 *__restrict__ W)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    const int Vh = g.Vh;
+    uint32_t tid = blockIdx.x * kBlock + threadIdx.x;
+    if (tid >= 2u * Vh) return;
+    int par = tid >= (uint32_t)Vh;
+    uint32_t h = tid - par * Vh;
+    uint32_t q, xh, y, z, t;
+    g.dxh.divmod(h, q, xh);
+    g.dy.divmod(q, q, y);
+    g.dz.divmod(q, t, z);
+    int x = 2 * xh + ((y + z + t + par) & 1);
+    long l = 2L * h + (x & 1);
+    double eta[4] = {1.0, (x & 1) ? -1.0 : 1.0, ((x + y) & 1) ? -1.0 : 1.0, ((x + y + z) & 1) ? -1.0 : 1.0};
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        double f = 0.5 * eta[mu];
+        if (mu == 3 && t == (uint32_t)g.Nt - 1) f = -f;
+        const double2 *u = U + (l * 4 + mu) * 9;
+        float2 *w = W + ((long)(par * 4 + mu) * 9) * Vh + h;
+#pragma unroll
+        for (int c = 0; c < 9; ++c) {
+            double2 v = u[c];
+            w[(long)c * Vh] = make_float2((float)(f * v.x), (float)(f * v.y));
+        }
+    }
+}
+
 // canonical parity vector [j][3] (j == h) -> planes [3][Vh], sites h0 <= h < h1
 __global__ void __launch_bounds__(kBlock)
 pack_kernel(int Vh, int h0, int h1, const double2 *__restrict__ canon, double2 *__restrict__ v)
@@ -96,6 +129,13 @@ int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, in
         launch_kernel(ingest_links_kernel<2>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W, not_su3);
     else
         launch_kernel(ingest_links_kernel<3>, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W, not_su3);
+    return 1;
+}
+
+int launch_ingest_links32(const Geom &g, const double *links_canon, float2 *W32, Launch L)
+{
+    int blocks = (2 * g.Vh + kBlock - 1) / kBlock;
+    launch_kernel(ingest_links32_kernel, blocks, kBlock, L.s, L.pdl, g, (const double2 *)links_canon, W32);
     return 1;
 }
 

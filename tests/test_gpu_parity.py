@@ -37,13 +37,15 @@ def q():
 class Rig:
     """One lattice: oracle + CUDA context fed the same canonical arrays."""
 
-    def __init__(self, torch, q, dims, mass, links, link_rows=3):
+    def __init__(self, torch, q, dims, mass, links, link_rows=3, mixed=False):
         self.torch, self.q = torch, q
         self.dims, self.mass = dims, mass
         self.lat = oracle.Lattice(dims, links)
         self.ctx = q.Context(dims, mass)
         if link_rows != 3:
             self.ctx.set_option(q.QCD_OPT_LINK_ROWS, link_rows)
+        if mixed:
+            self.ctx.set_option(q.QCD_OPT_MIXED, 1)
         # QCD_TEST_DSLASH_KERNEL=1 [QCD_TEST_DSLASH_PERSIST=n] runs the WHOLE suite on the bulk-staged kernel
         if os.environ.get("QCD_TEST_DSLASH_KERNEL"):
             self.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, int(os.environ["QCD_TEST_DSLASH_KERNEL"]))
@@ -258,6 +260,122 @@ def test_bulk_staged_kernel_in_the_solver(torch, q, persist):
     assert zero["status"] == 0 and zero["iterations"] == 0 and not zero["x"].any()
     cut = rig.solve(E, b, shifts, res, cfg.tol, max_iter=5)
     assert cut["status"] == 4 and cut["iterations"] == 5
+
+
+# ------------------------------------------------------------------ mixed precision (NEXT-3)
+
+def test_fp32_link_operator_is_the_oracle_operator_on_the_rounded_field(torch, q):
+    """QCD_OPT_OPERATOR_LINKS32: the inner operator of the mixed solver.  Links rounded to fp32, fp64
+    arithmetic: equal (1e-13) to the oracle's plain definition on the rounded field, and different from
+    the fp64 operator at the fp32 level."""
+    from oracle import mixed_precision as mp
+    dims, mass = (12, 6, 10, 4), 0.07
+    links = li.make_links(dims, "random", 11)
+    rig = Rig(torch, q, dims, mass, links, mixed=True)
+    lat32 = oracle.Lattice(dims, mp.round_links_fp32(links))
+    ve, vo = li.make_source(dims, 41, E), li.make_source(dims, 42, O)
+    full = (rig.dslash(O, ve), rig.mdagm(E, ve))
+    assert rel_l2(full[0], rig.lat.dslash(O, ve)) <= TOL_OP          # the fp64 path is untouched by the option
+    rig.ctx.set_option(q.QCD_OPT_OPERATOR_LINKS32, 1)
+    assert rel_l2(rig.dslash(O, ve), lat32.dslash(O, ve)) <= TOL_OP
+    assert rel_l2(rig.dslash(E, vo), lat32.dslash(E, vo)) <= TOL_OP
+    assert rel_l2(rig.mdagm(E, ve), lat32.mdagm(mass, E, ve)) <= TOL_OP
+    assert rel_l2(rig.mdagm(O, vo), lat32.mdagm(mass, O, vo)) <= TOL_OP
+    assert 1e-9 < rel_l2(rig.dslash(O, ve), full[0]) < 1e-6
+    rig.ctx.set_option(q.QCD_OPT_OPERATOR_LINKS32, 0)
+    assert np.array_equal(rig.dslash(O, ve), full[0])
+    plain = Rig(torch, q, dims, mass, links)                          # no fp32 copy loaded: refused
+    plain.ctx.set_option(q.QCD_OPT_OPERATOR_LINKS32, 1)
+    with pytest.raises(q.QcdError, match="QCD_ESTATE"):
+        plain.dslash(O, ve)
+
+
+@pytest.mark.parametrize("number,switch", [(1, 4), (2, 5), (1, 10)])
+def test_mixed_precision_solver_matches_the_oracle(torch, q, number, switch):
+    """QCD_OPT_MIXED: fp64 multishift to 10^-switch, then per-shift defect correction with the fp32-link
+    inner operator.  Same bars as the fp64 solver: recomputed fp64 residual <= 1.5 tol (here <= tol by
+    construction), every x_k and y within 1e-9 of the polished oracle; and within 1e-9 of the oracle's
+    own restatement of the mixed algorithm (oracle/mixed_precision.py)."""
+    from oracle import mixed_precision as mp
+    cfg, links, b, shifts, res = li.make_config_inputs(number)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links, mixed=True)
+    rig.ctx.set_option(q.QCD_OPT_MIXED_SWITCH_EXP, switch)
+    out = rig.solve(cfg.parity, b, shifts, res, cfg.tol)
+    exact = rig.lat.solve_exact(cfg.mass, cfg.parity, b, shifts, res, cfg.tol)
+    check_solve(rig, cfg, b, shifts, res, out, exact)
+    assert (out["true_res"] <= cfg.tol * (1 + 1e-9)).all()
+    ref = mp.mixed_precision_multishift(cfg.dims, links, cfg.mass, cfg.parity, b, shifts, res, cfg.tol,
+                                        switch_tol=10.0 ** -switch)
+    for k in range(len(shifts)):
+        assert rel_l2(out["x"][k], ref["x"][k]) <= TOL_X
+    total_ref = ref["stage1_iterations"] + int(ref["inner_iterations"].sum())
+    assert abs(out["iterations"] - total_ref) <= max(4, total_ref // 20), (out["iterations"], total_ref)
+    # without an x buffer (library workspace, sorted order) and with unsorted shifts: same answers
+    perm = np.argsort(-shifts)
+    out2 = rig.solve(cfg.parity, b, shifts[perm], res[perm], cfg.tol, own_x=False)
+    assert out2["status"] == 0 and rel_l2(out2["y"], exact["y"]) <= TOL_X
+    assert (out2["true_res"] <= cfg.tol * (1 + 1e-9)).all()
+    zero = rig.solve(E, np.zeros_like(b), shifts, res, cfg.tol)
+    assert zero["status"] == 0 and not zero["x"].any() and not zero["true_res"].any()
+
+
+def test_mixed_precision_light_mass(torch, q):
+    """kappa ~ 3e5: one round of the fp32-link inner solve gains about two digits only; the refinement
+    still lands on the fp64 solution."""
+    dims, mass, tol = (4, 4, 4, 4), 0.005, 1e-10
+    links = li.make_links(dims, "random", 5)
+    b = li.make_source(dims, 5, E)
+    shifts = np.logspace(-6, np.log10(4.0), 6)
+    rig = Rig(torch, q, dims, mass, links, mixed=True)
+    out = rig.solve(E, b, shifts, np.ones(6), tol)
+    assert out["status"] == 0 and (out["true_res"] <= tol * (1 + 1e-9)).all()
+    exact = rig.lat.solve_exact(mass, E, b, shifts, np.ones(6), tol)
+    for k in range(6):
+        assert rel_l2(out["x"][k], exact["x"][k]) <= TOL_X
+
+
+# ------------------------------------------------------------------ t-slab decomposition (NEXT-4, first half)
+
+@pytest.mark.parametrize("world,kernel", [(2, 0), (4, 0), (2, 1)])
+def test_slab_decomposition_on_one_gpu(torch, q, world, kernel):
+    """paper_1710_09178_b200/slab.py + qcd_dslash_range: every rank's slab, held with its two halo slices
+    as a lattice of its own, computed one after the other on this one GPU (no kernel waits on another).
+    Owned slices put together must EQUAL the single-context result bit for bit (same arithmetic per
+    site), and agree with the oracle's global operator; M^dag M needs a second halo fill."""
+    from paper_1710_09178_b200.slab import SlabPartition
+    dims, mass = (8, 6, 4, 8), 0.07
+    links = li.make_links(dims, "random", 3)
+    ve = li.make_source(dims, 41, E)
+    ref = Rig(torch, q, dims, mass, links)
+    ref.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, kernel)
+    want_d, want_a = ref.dslash(O, ve), ref.mdagm(E, ve)
+    parts = [SlabPartition(dims, world, r) for r in range(world)]
+    rigs = [Rig(torch, q, p.local_dims, mass, p.local_links(links)) for p in parts]
+    for r in rigs:
+        r.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, kernel)
+    lp_e, lp_o = SlabPartition.local_parity(E), SlabPartition.local_parity(O)
+    nt = dims[3]
+
+    def apply(global_in, out_parity_local, src_global=None, coeff=0.0):
+        """one slab-decomposed D: halos come from the global vector (what the exchange delivers)"""
+        pieces = []
+        for p, r in zip(parts, rigs):
+            d_in = r.to_internal(1 - out_parity_local, p.local_vector(global_in))
+            d_out = torch.full((r.ctx.vector_doubles,), np.nan, dtype=torch.float64, device="cuda")
+            d_src = None if src_global is None else r.to_internal(out_parity_local, p.local_vector(src_global))
+            r.ctx.dslash_range(out_parity_local, d_in, d_out, 1, p.nt_loc, d_src, coeff)
+            out = r.to_canonical(out_parity_local, d_out)
+            halo = out.reshape(p.nt_loc + 2, -1)[[0, -1]]
+            assert np.isnan(halo).all()                       # halo slices of the output are not touched
+            pieces.append(p.owned(out))
+        return np.concatenate(pieces)
+
+    got_d = apply(ve, lp_o)
+    assert np.array_equal(got_d, want_d) and rel_l2(got_d, ref.lat.dslash(O, ve)) <= TOL_OP
+    got_a = apply(got_d, lp_e, src_global=ve, coeff=mass * mass)          # m^2 v - D_eo (D_oe v)
+    assert np.array_equal(got_a, want_a) and rel_l2(got_a, ref.lat.mdagm(mass, E, ve)) <= TOL_OP
+    with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+        rigs[0].ctx.dslash_range(0, rigs[0].ctx.new_vector(), rigs[0].ctx.new_vector(), 1, nt)
 
 # ------------------------------------------------------------------ multishift CG
 
