@@ -123,6 +123,11 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     launches a persistent grid of n CTAs per SM that walk the tiles round-robin.
  *                     Dslash and M^dag M stay bit-identical; CG results change at rounding level only
  *                     (the <p,Ap> partial sums are added per CTA).
+ *   QCD_OPT_SWEEP_ALTERNATE  with 1, Dslash launches whose OUTPUT parity is even walk the lattice
+ *                     in descending order, the others in ascending order.  D_oe and D_eo read the same
+ *                     links, and inside M^dag M and the CG they alternate, so every apply starts on the
+ *                     links its predecessor touched last, which are the ones still in L2.  Dslash and
+ *                     M^dag M stay bit-identical.
  *   QCD_OPT_MIXED     (default 0) SURVEY 8(f) NEXT-3, the mixed-precision variant the paper sets aside
  *                     (PAPER.md:168).  With 1, the NEXT qcd_load_gauge also stores an fp32 copy of the
  *                     three-row links (+288 V bytes), and qcd_multishift_cg becomes: (1) the fp64
@@ -139,7 +144,8 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  * Returns QCD_EINVAL for an unknown option or a value out of range. */
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
        QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8,
-       QCD_OPT_MIXED = 9, QCD_OPT_MIXED_SWITCH_EXP = 10, QCD_OPT_OPERATOR_LINKS32 = 11 };
+       QCD_OPT_MIXED = 9, QCD_OPT_MIXED_SWITCH_EXP = 10, QCD_OPT_OPERATOR_LINKS32 = 11,
+       QCD_OPT_SWEEP_ALTERNATE = 12 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

@@ -17,12 +17,13 @@ import numpy as np
 QCD_EVEN, QCD_ODD = 0, 1
 QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH, QCD_OPT_LINK_ROWS, QCD_OPT_TGROUP = 0, 1, 2, 3, 4
 QCD_OPT_L2_PERSIST_MB, QCD_OPT_Y_ONLY, QCD_OPT_DSLASH_KERNEL, QCD_OPT_DSLASH_PERSIST = 5, 6, 7, 8
-QCD_OPT_MIXED, QCD_OPT_MIXED_SWITCH_EXP, QCD_OPT_OPERATOR_LINKS32 = 9, 10, 11
+QCD_OPT_MIXED, QCD_OPT_MIXED_SWITCH_EXP, QCD_OPT_OPERATOR_LINKS32, QCD_OPT_SWEEP_ALTERNATE = 9, 10, 11, 12
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONV, QCD_ESTATE = range(6)
 _STATUS_NAMES = ["QCD_OK", "QCD_EINVAL", "QCD_ENOMEM", "QCD_ECUDA", "QCD_ENOTCONV", "QCD_ESTATE"]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libqcd_b200.so")
+# QCD_B200_LIB: load another build of the same library (tuning aid: builds with different QCD_NVCC_EXTRA macros)
+_LIB_PATH = os.environ.get("QCD_B200_LIB") or os.path.join(_HERE, "libqcd_b200.so")
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "qcd.h")
 
 _vp, _ci, _cd, _cl = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_long

@@ -65,6 +65,7 @@ struct qcd_ctx {
     bool opt_operator_links32 = false;  // qcd_dslash / qcd_mdagm apply the fp32-link operator
     bool use_links32 = false;           // transient: the launches being enqueued use W32
     double2 *mx_r = nullptr, *mx_e = nullptr;
+    bool opt_sweep_alternate = false;   // Dslash launches with even output parity walk the tiles backwards
     int opt_dslash_kernel = 0;          // 0: register-staged links (dslash.cu); 1: bulk-copy staged (dslash_bulk.cu)
     int opt_dslash_persist = 0;         // bulk kernel: CTAs per SM of a persistent grid (0: one CTA per tile)
     // cached graph of one batch of CG iterations (valid for exactly the key below)
@@ -195,6 +196,7 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     DslashParams p{};
     p.W = c->W; p.link_rows = c->link_rows; p.in = in; p.out = out; p.out_parity = out_parity;
     p.W32 = c->W32; p.links32 = c->use_links32 ? 1 : 0;
+    p.reverse = c->opt_sweep_alternate && out_parity == QCD_EVEN ? 1 : 0;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->pap_partial;
@@ -409,6 +411,11 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         c->cg_cache.clear(); c->cg_exec = nullptr;
         return QCD_OK;
     case QCD_OPT_Y_ONLY: c->opt_y_only = value != 0; return QCD_OK;
+    case QCD_OPT_SWEEP_ALTERNATE:
+        c->opt_sweep_alternate = value != 0;
+        for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);   // baked into the captured launches
+        c->cg_cache.clear(); c->cg_exec = nullptr;
+        return QCD_OK;
     case QCD_OPT_MIXED: c->opt_mixed = value != 0; return QCD_OK;
     case QCD_OPT_MIXED_SWITCH_EXP:
         if (value < 1 || value > 15) return fail(c, QCD_EINVAL, "qcd_set_option: switch exponent must be in [1, 15]");
@@ -532,6 +539,7 @@ qcd_status qcd_dslash_range(qcd_ctx *c, int out_parity, const double *d_in, doub
     DslashParams p{};
     p.W = c->W; p.link_rows = c->link_rows; p.in = (const double2 *)d_in; p.out = (double2 *)d_out;
     p.out_parity = out_parity; p.src = (const double2 *)d_src; p.coeff = coeff;
+    p.reverse = c->opt_sweep_alternate && out_parity == QCD_EVEN ? 1 : 0;
     if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(g, p, c->Ld());
     return check_launch(c, "qcd_dslash_range");
@@ -903,7 +911,8 @@ qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, doubl
         g.t0 = i * nts; g.nt_run = nts;
         DslashParams p{};
         p.W = c->W; p.link_rows = c->link_rows; p.in = c->hv_a; p.out = c->hv_b; p.out_parity = out_parity;
-        c->launches += launch_dslash(g, p, c->Ld());
+        if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(g, p, c->opt_dslash_persist, c->Ld());
+        else c->launches += launch_dslash(g, p, c->Ld());
         c->launches += launch_unpack(c->g, c->hv_b, c->stage_out, c->L(), i * hs, (i + 1) * hs);
         QCD_CUDA(c, cudaEventRecord(ev_cmp[i], c->stream));
         QCD_CUDA(c, cudaStreamWaitEvent(c->s_out, ev_cmp[i], 0));

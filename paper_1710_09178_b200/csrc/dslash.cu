@@ -44,7 +44,7 @@ dslash_kernel(const Geom g, const DslashParams p)
     const WT *__restrict__ const W = sizeof(WT) == sizeof(float2) ? reinterpret_cast<const WT *>(p.W32)
                                                                  : reinterpret_cast<const WT *>(p.W);
     Site site;
-    locate<ROWS == 2>(g, p.out_parity, site);
+    locate_tile<ROWS == 2>(g, p.out_parity, p.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x, threadIdx.x, site);
     const bool valid = site.valid;
     const uint32_t h = site.h;
     const int par = p.out_parity;

@@ -71,10 +71,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
     } while (!ok);
 }
 // links are used once per apply: evict-first in L2, as the __ldcs of the register-staged kernel
+#ifndef QCD_BULK_L2_POLICY
+#define QCD_BULK_L2_POLICY "evict_first"     // tuning aid: "evict_normal", "evict_last"
+#endif
 __device__ __forceinline__ uint64_t evict_first_policy()
 {
     uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    asm volatile("createpolicy.fractional.L2::" QCD_BULK_L2_POLICY ".b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t pol)
@@ -139,7 +142,7 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
     const uint64_t pol = evict_first_policy();
     auto issue_one = [&]() {
         uint32_t t, sl0;
-        tile_origin(g, is.tile, t, sl0);
+        tile_origin(g, p.reverse ? ntiles - 1 - is.tile : is.tile, t, sl0);
         const int n = min(kTile, g.st - (int)sl0);
         const int h0 = (int)(t * (uint32_t)g.st + sl0);
         int lo, len;
@@ -182,7 +185,8 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
     } else {
         int stage = 0;
         uint32_t phase = 0;
-        for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        for (uint32_t seq = blockIdx.x; seq < ntiles; seq += gridDim.x) {
+            const uint32_t tile = p.reverse ? ntiles - 1 - seq : seq;
             Site site;
             locate_tile<ROWS == 2>(g, par, tile, threadIdx.x, site);
             const bool valid = site.valid;

@@ -144,6 +144,7 @@ struct DslashParams {
     const double2 *in;
     double2 *out;
     int out_parity;
+    int reverse;               // 1: the CTAs walk the tiles in descending order (QCD_OPT_SWEEP_ALTERNATE)
     // optional fused epilogue: out = coeff * src - D in     (src on out_parity); src == nullptr: out = D in
     const double2 *src;
     double coeff;              // used when coeff_from_state == 0

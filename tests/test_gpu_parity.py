@@ -473,6 +473,16 @@ def test_cta_order_option_does_not_change_a_single_bit(torch, q):
         s = rig.solve(E, ve, shifts, res, 1e-10)
         assert s["status"] == 0 and rel_l2(s["x"], sref["x"]) <= 1e-12
     assert rel_l2(ref[0], rig.lat.dslash(O, ve)) <= TOL_OP
+    # QCD_OPT_SWEEP_ALTERNATE: even-output launches walk the tiles backwards; same bits for the operators
+    for kern in (0, 1):
+        rig.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, kern)
+        rig.ctx.set_option(q.QCD_OPT_SWEEP_ALTERNATE, 1)
+        out = (rig.dslash(O, ve), rig.dslash(E, vo), rig.mdagm(E, ve))
+        assert all(np.array_equal(a, b) for a, b in zip(out, ref))
+        s = rig.solve(E, ve, shifts, res, 1e-10)
+        assert s["status"] == 0 and rel_l2(s["x"], sref["x"]) <= 1e-12
+        rig.ctx.set_option(q.QCD_OPT_SWEEP_ALTERNATE, 0)
+    rig.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, 0)
     with pytest.raises(q.QcdError, match="QCD_EINVAL"):
         rig.ctx.set_option(q.QCD_OPT_TGROUP, -1)
     # L2 persisting window: applies at the next load, results unchanged
