@@ -231,6 +231,13 @@ def oracle_sample(cfg, links, b, shifts, res, dslash_seconds: float = 6.0, cg_se
         if t_d >= dslash_seconds:
             break
     del ve
+    # the same pair on ONE thread ("for Dslash only, also with 1 thread")
+    nthreads = oracle.threads()
+    oracle.set_threads(1)
+    t0 = time.perf_counter()
+    lat.dslash(0, lat.dslash(1, b))
+    t_1 = (time.perf_counter() - t0) / 2
+    oracle.set_threads(nthreads)
     gbps = 2 * n_pairs * dslash_bytes(cfg.volume) / t_d / 1e9
     t0 = time.perf_counter()
     probe = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=3, want_x=False)
@@ -239,7 +246,7 @@ def oracle_sample(cfg, links, b, shifts, res, dslash_seconds: float = 6.0, cg_se
     t0 = time.perf_counter()
     out = lat.multishift_cg(cfg.mass, cfg.parity, b, shifts, res, cfg.tol, max_iter=iters, want_x=False)
     t_cg = time.perf_counter() - t0
-    return dict(gbps=gbps, dslash_s=t_d / (2 * n_pairs), pairs=n_pairs,
+    return dict(gbps=gbps, dslash_s=t_d / (2 * n_pairs), dslash_s_1thread=t_1, pairs=n_pairs,
                 cg_s_per_iter=t_cg / max(out["iterations"], 1), cg_iters=out["iterations"],
                 cg_converged=out["status"] == 0, cg_seconds=t_cg,
                 cores=oracle.threads(), seconds=t_d + t_cg)
@@ -773,7 +780,8 @@ def main():
                           f"iterations of the {cfg.nshift}-shift CG"
                           f"{' (the whole solve)' if smp['cg_converged'] else ''} "
                           f"({smp['seconds']:.1f} s of host time)",
-                "dslash_us_per_apply": 1e6 * smp["dslash_s"], "cg_s_per_iteration": smp["cg_s_per_iter"],
+                "dslash_us_per_apply": 1e6 * smp["dslash_s"], "dslash_us_per_apply_1_thread": 1e6 * smp["dslash_s_1thread"],
+                "cg_s_per_iteration": smp["cg_s_per_iter"],
                 "cg_s_sampled": smp["cg_seconds"], "cg_converged_in_sample": smp["cg_converged"],
                 "host_cpu_count": os.cpu_count()}
         print(json.dumps(line), flush=True)

@@ -85,9 +85,19 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     launches after convergence, no host polling.  Measured on B200 it is no faster
  *                     than 1 (7.93 vs 7.84 ms at 32^3x8, 5.69 vs 5.31 ms at 4^4): the loop node costs
  *                     about 1 us per iteration and breaks the PDL chain between iterations.
- *   QCD_OPT_CG_BATCH  (default 8) iterations per batch; the host reads the device's convergence flag
+ *   QCD_OPT_CG_BATCH  (default 8) iterations per batch (per body of the device-side loop: QCD_OPT_CG_DEFER
+ *                     iterations); the host reads the device's convergence flag
  *                     once per batch, one batch late, so up to 2 batches of early-exit kernels follow
  *                     convergence.  1 <= value <= 1024.
+ *   QCD_OPT_CG_DEFER  (default 8) deferred shift updates.  Inside the iteration only p_0 of the base system
+ *                     is needed (the next M^dag M acts on it); x_k and p_k of the shifts k >= 1 are
+ *                     needed at the end.  With value m > 1 the per-iteration update touches the base
+ *                     shift only, the last m residuals are kept in a ring, and every m iterations ONE
+ *                     pass applies the m stored updates to x_k, p_k of all other shifts: those vectors
+ *                     move once per m iterations instead of once per iteration (96 V/m bytes per shift
+ *                     and iteration instead of 96 V).  Every element sees the same operations in the
+ *                     same order: results are bit-identical to value 1 (update every iteration).
+ *                     1 <= value <= 8.  Not used by the y-only form and single-shift solves.
  *   QCD_OPT_TGROUP    (default 0 = chosen by the library) order in which the Dslash CTAs walk the
  *                     lattice: groups of this many 128-site chunks of a t-slice are processed for all t
  *                     before the next group starts, so +-t neighbours are reused out of L2.  Dslash and
@@ -123,11 +133,13 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     launches a persistent grid of n CTAs per SM that walk the tiles round-robin.
  *                     Dslash and M^dag M stay bit-identical; CG results change at rounding level only
  *                     (the <p,Ap> partial sums are added per CTA).
- *   QCD_OPT_SWEEP_ALTERNATE  with 1, Dslash launches whose OUTPUT parity is even walk the lattice
- *                     in descending order, the others in ascending order.  D_oe and D_eo read the same
- *                     links, and inside M^dag M and the CG they alternate, so every apply starts on the
- *                     links its predecessor touched last, which are the ones still in L2.  Dslash and
- *                     M^dag M stay bit-identical.
+ *   QCD_OPT_SWEEP_ALTERNATE  (default 2 = auto) 1: Dslash launches whose OUTPUT parity is even walk the
+ *                     lattice in descending order, the others in ascending order, and the links are
+ *                     loaded with the ordinary instead of the streaming policy.  D_oe and D_eo read the
+ *                     same links, and inside M^dag M and the CG they alternate, so every apply starts on
+ *                     the links its predecessor touched last, which are still in L2.  0: one direction,
+ *                     streaming loads.  2: on when the stored links are at most twice the size of L2
+ *                     (decided at qcd_load_gauge).  Dslash and M^dag M stay bit-identical.
  *   QCD_OPT_MIXED     (default 0) SURVEY 8(f) NEXT-3, the mixed-precision variant the paper sets aside
  *                     (PAPER.md:168).  With 1, the NEXT qcd_load_gauge also stores an fp32 copy of the
  *                     three-row links (+288 V bytes), and qcd_multishift_cg becomes: (1) the fp64
@@ -145,7 +157,7 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
        QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8,
        QCD_OPT_MIXED = 9, QCD_OPT_MIXED_SWITCH_EXP = 10, QCD_OPT_OPERATOR_LINKS32 = 11,
-       QCD_OPT_SWEEP_ALTERNATE = 12 };
+       QCD_OPT_SWEEP_ALTERNATE = 12, QCD_OPT_CG_DEFER = 13 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

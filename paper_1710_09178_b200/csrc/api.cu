@@ -56,7 +56,10 @@ struct qcd_ctx {
     int opt_cg_graph = 1;               // 0: plain launches; 1: one captured graph per batch; 2: device-side WHILE loop
     unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
     bool opt_y_only = false;            // qcd_inv_sqrt / qcd_apply_pow accumulate y directly, no x_k
-    int opt_cg_batch = 8;               // iterations enqueued per batch / per graph
+    int opt_cg_batch = 8;               // iterations enqueued per batch / per graph (rounded up to a multiple of defer)
+    int opt_cg_defer = kMaxDefer;       // QCD_OPT_CG_DEFER: iterations per deferred update of the shifts k >= 1
+    int cur_defer = 1;                  // the value the solve being enqueued uses (1 for y-only and single-shift solves)
+    int r_slots = 0;                    // vectors allocated in the residual ring c->r
     // NEXT-3 (mixed precision): fp32 copy of the three-row links and the buffers of the refinement
     float2 *W32 = nullptr;
     bool links32_loaded = false;
@@ -65,17 +68,20 @@ struct qcd_ctx {
     bool opt_operator_links32 = false;  // qcd_dslash / qcd_mdagm apply the fp32-link operator
     bool use_links32 = false;           // transient: the launches being enqueued use W32
     double2 *mx_r = nullptr, *mx_e = nullptr;
-    bool opt_sweep_alternate = false;   // Dslash launches with even output parity walk the tiles backwards
+    int opt_sweep_alternate = 2;        // 0 off, 1 on, 2 auto (on when the links are at most twice the size of L2)
+    bool sweep_on = false;              // decided at qcd_load_gauge: even-output Dslash launches walk the tiles
+                                        // backwards and the links are loaded with the ordinary (keep) policy
+    size_t l2_bytes = 0;
     int opt_dslash_kernel = 0;          // 0: register-staged links (dslash.cu); 1: bulk-copy staged (dslash_bulk.cu)
     int opt_dslash_persist = 0;         // bulk kernel: CTAs per SM of a persistent grid (0: one CTA per tile)
     // cached graph of one batch of CG iterations (valid for exactly the key below)
     cudaGraphExec_t cg_exec = nullptr;  // the entry of cg_cache selected by the last ensure_cg_graph
     cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
     struct CgKey {
-        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0; bool pdl = false, apw = false, yonly = false, l32 = false; double mass = 0.0;
+        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0, defer = 0; bool pdl = false, apw = false, yonly = false, l32 = false; double mass = 0.0;
         const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
         bool operator==(const CgKey &o) const {
-            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && pdl == o.pdl && apw == o.apw && yonly == o.yonly && l32 == o.l32 && mass == o.mass &&
+            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && defer == o.defer && pdl == o.pdl && apw == o.apw && yonly == o.yonly && l32 == o.l32 && mass == o.mass &&
                    x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
         }
     };
@@ -150,6 +156,20 @@ void setup_l2_window(qcd_ctx *c)
     c->apw_on = true;
 }
 
+// QCD_OPT_SWEEP_ALTERNATE.  D_oe and D_eo read the SAME links (each reads the forward links of its output
+// parity and the backward links of the other), and inside M^dag M, the CG and any power iteration they
+// alternate.  On a gauge field of about the size of L2, walking the lattice in ascending order for odd
+// outputs and in descending order for even outputs lets every apply start on the links its predecessor
+// touched last -- still in L2 if they were loaded with the ordinary policy -- where a one-directional
+// sweep over more than L2 holds finds nothing of itself (LRU).  Measured at 32^3x8 (151 MB of links,
+// 126 MB of L2): 20.6 -> 18.1 us per apply, two-row (100 MB) 14.8 -> 13.5, solve 7.19 -> 6.95 ms; at
+// 48^3x12 (764 MB) and 64^3x16 (2.4 GB) nothing to win, and the streaming policy is the better one there.
+void decide_sweep(qcd_ctx *c)
+{
+    const size_t link_bytes = (size_t)c->g.Vh * 2 * 4 * 3 * c->link_rows * sizeof(double2);
+    c->sweep_on = c->opt_sweep_alternate == 1 || (c->opt_sweep_alternate == 2 && link_bytes <= 2 * c->l2_bytes);
+}
+
 bool bad_parity(int p) { return p != QCD_EVEN && p != QCD_ODD; }
 
 // every device buffer is accessed with 16-byte loads and stores (double2)
@@ -172,7 +192,12 @@ qcd_status ensure_host_staging(qcd_ctx *c)
 qcd_status ensure_cg_workspace(qcd_ctx *c, int nshift, bool need_x)
 {
     if (!c->q) QCD_CUDA(c, dev_alloc(&c->q, (size_t)c->n2));
-    if (!c->r) QCD_CUDA(c, dev_alloc(&c->r, (size_t)c->n2));
+    if (c->r_slots < kMaxDefer) {          // the residual ring (deferred shift updates, blas.cu)
+        if (c->r) cudaFree(c->r);
+        c->r = nullptr; c->r_slots = 0;
+        QCD_CUDA(c, dev_alloc(&c->r, (size_t)c->n2 * kMaxDefer));
+        c->r_slots = kMaxDefer;
+    }
     if (c->p_cap < nshift) {
         if (c->p) cudaFree(c->p);
         c->p = nullptr; c->p_cap = 0;
@@ -196,7 +221,8 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     DslashParams p{};
     p.W = c->W; p.link_rows = c->link_rows; p.in = in; p.out = out; p.out_parity = out_parity;
     p.W32 = c->W32; p.links32 = c->use_links32 ? 1 : 0;
-    p.reverse = c->opt_sweep_alternate && out_parity == QCD_EVEN ? 1 : 0;
+    p.reverse = c->sweep_on && out_parity == QCD_EVEN ? 1 : 0;
+    p.keep_links = c->sweep_on ? 1 : 0;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->pap_partial;
@@ -206,7 +232,9 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     return QCD_OK;
 }
 
-// one multishift-CG iteration: 4 kernels, all scalars stay on the device
+// one multishift-CG iteration: 4 kernels, all scalars stay on the device.  With deferred
+// shift updates (cur_defer > 1) the fourth kernel updates the base shift only; the caller enqueues
+// enqueue_cg_flush after every cur_defer-th iteration.
 void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
 {
     // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
@@ -218,7 +246,24 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
     if (y_only)      // `x` is the single vector y
         c->launches += launch_cg_update_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
     else
-        c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
+        c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->cur_defer > 1 ? 1 : 0, c->L());
+}
+
+// the deferred updates of the shifts k >= 1 for the last `window` enqueued iterations
+void enqueue_cg_flush(qcd_ctx *c, double2 *x, int window)
+{
+    c->launches += launch_cg_flush_shifts(c->n2, c->r, x, c->p, c->n2, c->st, window, c->L());
+}
+
+// `count` iterations with the flushes that belong to them (count is a multiple of cur_defer, or the tail
+// of a solve enqueued without graphs)
+void enqueue_cg_iterations(qcd_ctx *c, int parity, double2 *x, bool y_only, int count)
+{
+    const int m = c->cur_defer;
+    for (int i = 1; i <= count; ++i) {
+        enqueue_cg_iteration(c, parity, x, y_only);
+        if (m > 1 && (i % m == 0 || i == count)) enqueue_cg_flush(c, x, i % m == 0 ? m : i % m);
+    }
 }
 
 // Capture `batch` iterations into a graph (once per distinct set of buffers, parity and mass);
@@ -226,7 +271,7 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
 qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y_only)
 {
     qcd_ctx::CgKey key;
-    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.kern = c->opt_dslash_kernel; key.persist = c->opt_dslash_persist; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
+    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.kern = c->opt_dslash_kernel; key.persist = c->opt_dslash_persist; key.defer = c->cur_defer; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
     key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp; key.l32 = c->use_links32;
     for (auto &e : c->cg_cache)
         if (e.key == key) { c->cg_exec = e.exec; return QCD_OK; }
@@ -241,7 +286,7 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y
     if (batch > 0) {
         e = cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal);
         if (e == cudaSuccess) {
-            for (int i = 0; i < batch; ++i) enqueue_cg_iteration(c, parity, x, y_only);
+            enqueue_cg_iterations(c, parity, x, y_only, batch);
             cudaGraph_t graph = nullptr;
             e = cudaStreamEndCapture(c->cap_stream, &graph);
             if (e == cudaSuccess) e = cudaGraphInstantiate(&c->cg_exec, graph, 0);
@@ -267,7 +312,7 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y
             e = cudaStreamBeginCaptureToGraph(c->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
             if (e == cudaSuccess) {
                 c->loop_handle = (unsigned long long)handle;
-                enqueue_cg_iteration(c, parity, x, y_only);
+                enqueue_cg_iterations(c, parity, x, y_only, c->cur_defer);     // body: defer iterations + their flush
                 c->loop_handle = 0;
                 cudaGraph_t same = nullptr;
                 e = cudaStreamEndCapture(c->cap_stream, &same);
@@ -319,6 +364,7 @@ qcd_status qcd_create(const int dims[4], double mass, void *cuda_stream, qcd_ctx
     qcd_ctx *c = new (std::nothrow) qcd_ctx;
     if (!c) return fail(nullptr, QCD_ENOMEM, "qcd_create: host allocation failed");
     c->device = dev;
+    c->l2_bytes = (size_t)prop.l2CacheSize;
     c->mass = mass;
     c->stream = (cudaStream_t)cuda_stream;
     Geom &g = c->g;
@@ -404,6 +450,10 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         if (value < 1 || value > 1024) return fail(c, QCD_EINVAL, "qcd_set_option: batch must be in [1, 1024]");
         c->opt_cg_batch = (int)value;
         return QCD_OK;
+    case QCD_OPT_CG_DEFER:
+        if (value < 1 || value > kMaxDefer) return fail(c, QCD_EINVAL, "qcd_set_option: defer must be in [1, 8]");
+        c->opt_cg_defer = (int)value;
+        return QCD_OK;
     case QCD_OPT_TGROUP:
         if (value < 0) return fail(c, QCD_EINVAL, "qcd_set_option: tgroup must be >= 0");
         c->g.tgroup = value == 0 ? auto_tgroup(c->g) : value > c->g.chunks ? c->g.chunks : (int)value;
@@ -412,7 +462,9 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         return QCD_OK;
     case QCD_OPT_Y_ONLY: c->opt_y_only = value != 0; return QCD_OK;
     case QCD_OPT_SWEEP_ALTERNATE:
-        c->opt_sweep_alternate = value != 0;
+        if (value < 0 || value > 2) return fail(c, QCD_EINVAL, "qcd_set_option: sweep mode must be 0, 1 or 2");
+        c->opt_sweep_alternate = (int)value;
+        decide_sweep(c);
         for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);   // baked into the captured launches
         c->cg_cache.clear(); c->cg_exec = nullptr;
         return QCD_OK;
@@ -471,7 +523,7 @@ qcd_status qcd_load_gauge(qcd_ctx *c, const double *d_links)
         if ((s = check_launch(c, "qcd_load_gauge (fp32 copy)")) != QCD_OK) return s;
         c->links32_loaded = true;
     }
-    c->gauge_loaded = true; c->link_rows = c->opt_link_rows; setup_l2_window(c);
+    c->gauge_loaded = true; c->link_rows = c->opt_link_rows; setup_l2_window(c); decide_sweep(c);
     c->fresh_gauge = true;
     return QCD_OK;
 }
@@ -539,7 +591,8 @@ qcd_status qcd_dslash_range(qcd_ctx *c, int out_parity, const double *d_in, doub
     DslashParams p{};
     p.W = c->W; p.link_rows = c->link_rows; p.in = (const double2 *)d_in; p.out = (double2 *)d_out;
     p.out_parity = out_parity; p.src = (const double2 *)d_src; p.coeff = coeff;
-    p.reverse = c->opt_sweep_alternate && out_parity == QCD_EVEN ? 1 : 0;
+    p.reverse = c->sweep_on && out_parity == QCD_EVEN ? 1 : 0;
+    p.keep_links = c->sweep_on ? 1 : 0;
     if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(g, p, c->Ld());
     return check_launch(c, "qcd_dslash_range");
@@ -611,6 +664,11 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     h.alpha_old = 1.0; h.beta_old = 0.0;
     h.tol = tol; h.freeze = 0.1;
     h.nshift = nshift; h.max_iter = max_iter;
+    // deferred updates of the shifts k >= 1 (blas.cu): not for the y-only form (it keeps no x_k) and
+    // pointless for a single shift
+    const int defer = (y_only || nshift == 1) ? 1 : std::max(1, std::min(c->opt_cg_defer, kMaxDefer));
+    h.defer = defer;
+    c->cur_defer = defer;
     std::vector<long long> xoff_caller(nshift);
     for (int k = 0; k < nshift; ++k) {
         h.sigma[k] = shifts[order[k]];
@@ -623,7 +681,8 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     h.sigma0 = h.sigma[0];
     QCD_CUDA(c, cudaMemcpyAsync(c->st, &h, sizeof h, cudaMemcpyHostToDevice, st));
     QCD_CUDA(c, cudaMemsetAsync(x, 0, (size_t)n2 * (y_only ? 1 : nshift) * sizeof(double2), st));
-    c->launches += launch_cg_init(n2, b, c->r, c->p, n2, nshift, c->partial, c->st, c->L());
+    // the initial residual b is slot defer - 1 of the ring: "r after iteration 0"
+    c->launches += launch_cg_init(n2, b, c->r + (long)(defer - 1) * n2, c->p, n2, nshift, c->partial, c->st, c->L());
 
     // iteration loop: enqueue only (one graph replay, or 4 launches per iteration, per batch)
     const int batch = std::max(1, std::min(c->opt_cg_batch, max_iter));
@@ -641,9 +700,9 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         const int nb = use_graph ? batch : std::min(batch, max_iter - enq);
         if (use_graph) {
             QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));
-            c->launches += 4L * batch;
+            c->launches += 4L * batch + (defer > 1 ? (batch + defer - 1) / defer : 0);
         } else {
-            for (int i = 0; i < nb; ++i) enqueue_cg_iteration(c, parity, x, y_only);
+            enqueue_cg_iterations(c, parity, x, y_only, nb);
         }
         enq += nb;
         if (pending) {
@@ -690,7 +749,10 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     QCD_CUDA(c, cudaStreamSynchronize(st));
 
     *iterations = h.iter;
-    if (c->opt_cg_graph == 2) c->launches += 4L * std::max(h.iter, 1);   // the loop body ran once per iteration
+    if (c->opt_cg_graph == 2) {          // the loop body (defer iterations and their flush) ran ceil(iter/defer) times
+        const long bodies = std::max((h.iter + defer - 1) / defer, 1);
+        c->launches += bodies * (4L * defer + (defer > 1 ? 1 : 0));
+    }
     const double rho_b = h.rho_b;
     for (int k = 0; k < nshift; ++k)
         true_res[k] = rho_b > 0.0 ? std::sqrt(c->h_results[k] / rho_b) : 0.0;

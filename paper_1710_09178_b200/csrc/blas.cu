@@ -53,12 +53,13 @@ constexpr int kRMaxBlocks = 148 * 4;
 
 template <bool LOOP>
 __global__ void __launch_bounds__(kBlock)
-cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__ q,
+cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
                    const double *__restrict__ pap_partial, int npap, double *partial, CgState *st,
                    cudaGraphConditionalHandle loop)
 {
     pdl_wait();
     pdl_launch_dependents();
+    if (blockIdx.x == 0 && threadIdx.x == 0) st->enq += 1;     // read by the flush kernel only
     if (st->done) {                       // dead iteration after convergence
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             st->done_prev = 1;
@@ -66,6 +67,11 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
         }
         return;
     }
+    // this is iteration n = st->iter + 1 (st->iter is advanced by the last block only, after every CTA has
+    // read it): r_{n-1} is ring slot (n - 2) mod defer, r_n goes to slot (n - 1) mod defer
+    const int m = st->defer, it = st->iter;
+    const double2 *rin = ring + (long)((it + m - 1) % m) * n2;     // == r when defer == 1: no __restrict__
+    double2 *r = ring + (long)(it % m) * n2;
     double t = 0.0;
     for (int i = threadIdx.x; i < npap; i += kBlock) t += __ldcg(pap_partial + i);
     const double pAp = block_sum<kBlock>(t);
@@ -76,7 +82,7 @@ cg_update_r_kernel(long n2, double2 *__restrict__ r, const double2 *__restrict__
 #pragma unroll
         for (int e = 0; e < kRUnroll; ++e) {
             const long i = base + (long)e * kBlock;
-            if (i < n2) { rv[e] = r[i]; qv[e] = __ldg(q + i); }
+            if (i < n2) { rv[e] = rin[i]; qv[e] = __ldg(q + i); }
         }
 #pragma unroll
         for (int e = 0; e < kRUnroll; ++e) {
@@ -110,17 +116,18 @@ constexpr int kShiftUnroll = 4;
 constexpr int kShiftChunk = kBlock * kShiftUnroll;
 
 __global__ void __launch_bounds__(kBlock)
-cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restrict__ x,
-                        double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
+cg_update_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__restrict__ x,
+                        double2 *__restrict__ p, long pstride, const CgState *__restrict__ st, int base_only)
 {
     pdl_wait();
     pdl_launch_dependents();
     if (st->done_prev) return;
     __shared__ double s_a[kMaxShifts], s_z[kMaxShifts], s_b[kMaxShifts];
     __shared__ long long s_x[kMaxShifts], s_p[kMaxShifts];
-    const int nl = st->nlist;
+    const double2 *__restrict__ r = ring + (long)((st->iter - 1) % st->defer) * n2;   // r of the iteration just done
+    const int nl = base_only ? 1 : st->nlist;       // base_only: the shifts k >= 1 are updated by the flush kernel
     if (threadIdx.x < nl) {
-        const int k = st->list[threadIdx.x];
+        const int k = base_only ? 0 : st->list[threadIdx.x];
         s_a[threadIdx.x] = st->coef_a[k];
         s_z[threadIdx.x] = st->coef_z[k];
         s_b[threadIdx.x] = st->coef_b[k];
@@ -157,18 +164,122 @@ cg_update_shifts_kernel(long n2, const double2 *__restrict__ r, double2 *__restr
     }
 }
 
+// Deferred updates of the shifts k >= 1.  Only p_0 is needed inside the iteration (the next matvec acts
+// on it); x_k and p_k of the other shifts are needed at the end.  So their updates
+//     x_k += alpha_k^(n) p_k ;  p_k = zeta_k^(n) r_n + beta_k^(n) p_k          n = lo + 1 .. hi
+// are applied in ONE pass per `defer` iterations from the stored coefficients (CgState::hist_*) and the
+// ring of the last `defer` residuals: x_k and p_k then move once per defer iterations instead of once
+// per iteration, 96 V/defer bytes per shift and iteration instead of 96 V -- the traffic of "the heaviest
+// kernel which updates three large arrays" divided by defer.  Every element sees exactly
+// the operations of the undeferred kernel in the same order: the results are bit-identical.
+// The kernel flushes the iterations (enq - window, min(enq, iter)]: enq counts the enqueued iterations
+// (dead ones included), iter the executed ones; neither is written while this kernel runs.
+constexpr int kFlushBlock = 256;
+
+__global__ void __launch_bounds__(kFlushBlock)
+cg_flush_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__restrict__ x,
+                       double2 *__restrict__ p, long pstride, const CgState *__restrict__ st, int window)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    const int m = st->defer;
+    const int lo = st->enq - window, hi = min(st->enq, st->iter);
+    const int cnt = hi - lo;                       // iterations lo + 1 .. hi, 0 <= cnt <= window <= m
+    if (cnt <= 0) return;
+    __shared__ double s_a[kMaxDefer][kMaxShifts], s_z[kMaxDefer][kMaxShifts], s_b[kMaxDefer][kMaxShifts];
+    __shared__ long long s_x[kMaxShifts], s_p[kMaxShifts];
+    __shared__ int s_steps[kMaxShifts];            // leading iterations of the window shift j takes part in
+    __shared__ int s_n;
+    __shared__ int s_all[kMaxShifts], s_map[kMaxShifts];
+    const int ns = st->nshift;
+    if (threadIdx.x < kMaxShifts) {                // thread k: how many leading iterations of the window shift k is in
+        const int k = threadIdx.x;
+        int steps = 0;                             // activity only ever ends: a prefix of the window
+        if (k >= 1 && k < ns)
+            while (steps < cnt && st->hist_on[(lo + steps) % m][k]) ++steps;
+        s_all[k] = steps;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {                        // compact: the shifts that have anything to do
+        int nl = 0;
+        for (int k = 1; k < ns; ++k)
+            if (s_all[k] > 0) {
+                s_map[nl] = k;
+                s_steps[nl] = s_all[k];
+                s_x[nl] = st->xoff[k];
+                s_p[nl] = (long long)k * pstride;
+                ++nl;
+            }
+        s_n = nl;
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < cnt * s_n; idx += kFlushBlock) {
+        const int j = idx / s_n, l = idx - j * s_n, k = s_map[l], slot = (lo + j) % m;
+        s_a[j][l] = st->hist_a[slot][k];           // slots beyond a shift's last step are never used
+        s_z[j][l] = st->hist_z[slot][k];
+        s_b[j][l] = st->hist_b[slot][k];
+    }
+    __syncthreads();
+    const int nl = s_n;
+    if (nl == 0) return;
+    for (long i = (long)blockIdx.x * kFlushBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kFlushBlock) {
+        double2 rv[kMaxDefer];
+#pragma unroll
+        for (int j = 0; j < kMaxDefer; ++j)
+            if (j < cnt) rv[j] = __ldg(ring + (long)((lo + j) % m) * n2 + i);
+        int l = 0;
+        for (; l + 1 < nl; l += 2) {                // two shifts in flight per thread
+            double2 *xa = x + s_x[l] + i, *pa = p + s_p[l] + i, *xb = x + s_x[l + 1] + i, *pb = p + s_p[l + 1] + i;
+            double2 xva = *xa, pva = *pa, xvb = *xb, pvb = *pb;
+            const int sa = s_steps[l], sb = s_steps[l + 1];
+#pragma unroll
+            for (int j = 0; j < kMaxDefer; ++j) {
+                if (j < sa) {
+                    xva.x = fma(s_a[j][l], pva.x, xva.x);
+                    xva.y = fma(s_a[j][l], pva.y, xva.y);
+                    pva.x = fma(s_b[j][l], pva.x, s_z[j][l] * rv[j].x);
+                    pva.y = fma(s_b[j][l], pva.y, s_z[j][l] * rv[j].y);
+                }
+                if (j < sb) {
+                    xvb.x = fma(s_a[j][l + 1], pvb.x, xvb.x);
+                    xvb.y = fma(s_a[j][l + 1], pvb.y, xvb.y);
+                    pvb.x = fma(s_b[j][l + 1], pvb.x, s_z[j][l + 1] * rv[j].x);
+                    pvb.y = fma(s_b[j][l + 1], pvb.y, s_z[j][l + 1] * rv[j].y);
+                }
+            }
+            *xa = xva; *pa = pva; *xb = xvb; *pb = pvb;
+        }
+        if (l < nl) {
+            double2 *xa = x + s_x[l] + i, *pa = p + s_p[l] + i;
+            double2 xva = *xa, pva = *pa;
+            const int sa = s_steps[l];
+#pragma unroll
+            for (int j = 0; j < kMaxDefer; ++j) {
+                if (j < sa) {
+                    xva.x = fma(s_a[j][l], pva.x, xva.x);
+                    xva.y = fma(s_a[j][l], pva.y, xva.y);
+                    pva.x = fma(s_b[j][l], pva.x, s_z[j][l] * rv[j].x);
+                    pva.y = fma(s_b[j][l], pva.y, s_z[j][l] * rv[j].y);
+                }
+            }
+            *xa = xva; *pa = pva;
+        }
+    }
+}
+
 // y-only form of the shift update (QCD_OPT_Y_ONLY): when only y = sum_k c_k x_k is wanted (eq. 8,
 // the heat bath and the action need (M^dag M)^(1/b) phi, not the x_k), the x_k never
 // have to exist: x_k += alpha_k p_k turns into y += c_k alpha_k p_k, accumulated in registers over the
 // active shifts of an element.  Per active shift the kernel then moves p_k in and out (48 V bytes)
 // instead of x_k and p_k (96 V bytes); r and y once per element.
 __global__ void __launch_bounds__(kBlock)
-cg_update_shifts_y_kernel(long n2, const double2 *__restrict__ r, double2 *__restrict__ y,
+cg_update_shifts_y_kernel(long n2, const double2 *__restrict__ ring, double2 *__restrict__ y,
                           double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
 {
     pdl_wait();
     pdl_launch_dependents();
     if (st->done_prev) return;
+    const double2 *__restrict__ r = ring + (long)((st->iter - 1) % st->defer) * n2;
     __shared__ double s_ca[kMaxShifts], s_z[kMaxShifts], s_b[kMaxShifts];
     __shared__ long long s_p[kMaxShifts];
     const int nl = st->nlist;
@@ -296,35 +407,44 @@ int cg_update_r_grid_blocks(long n2)
     return (int)(b < kRMaxBlocks ? (b > 0 ? b : 1) : kRMaxBlocks);
 }
 
-int launch_cg_update_r(long n2, double2 *r, const double2 *q, const double *pap_partial, int npap,
+int launch_cg_update_r(long n2, double2 *ring, const double2 *q, const double *pap_partial, int npap,
                        double *partial, CgState *st, unsigned long long loop_handle, Launch L)
 {
     const int grid = cg_update_r_grid_blocks(n2);
     if (loop_handle)
-        launch_kernel(cg_update_r_kernel<true>, grid, kBlock, L.s, L.pdl, n2, r, q, pap_partial, npap, partial, st,
+        launch_kernel(cg_update_r_kernel<true>, grid, kBlock, L.s, L.pdl, n2, ring, q, pap_partial, npap, partial, st,
                       (cudaGraphConditionalHandle)loop_handle);
     else
-        launch_kernel(cg_update_r_kernel<false>, grid, kBlock, L.s, L.pdl, n2, r, q, pap_partial, npap, partial, st,
+        launch_kernel(cg_update_r_kernel<false>, grid, kBlock, L.s, L.pdl, n2, ring, q, pap_partial, npap, partial, st,
                       (cudaGraphConditionalHandle)0);
     return 1;
 }
 
-int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
-                            CgState *st, Launch L)
+int launch_cg_update_shifts(long n2, const double2 *ring, double2 *x, double2 *p, long pstride,
+                            CgState *st, int base_only, Launch L)
 {
     // the number of active shifts is only known on the device: size the grid for all of them
-    long units = (n2 + kShiftChunk - 1) / kShiftChunk * kMaxShifts;
+    long units = (n2 + kShiftChunk - 1) / kShiftChunk * (base_only ? 1 : kMaxShifts);
     int grid = (int)(units < 148 * 8 ? (units > 0 ? units : 1) : 148 * 8);
-    launch_kernel(cg_update_shifts_kernel, grid, kBlock, L.s, L.pdl, n2, r, x, p, pstride, st);
+    launch_kernel(cg_update_shifts_kernel, grid, kBlock, L.s, L.pdl, n2, ring, x, p, pstride, st, base_only);
     return 1;
 }
 
-int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p, long pstride,
+int launch_cg_flush_shifts(long n2, const double2 *ring, double2 *x, double2 *p, long pstride,
+                           const CgState *st, int window, Launch L)
+{
+    long blocks = (n2 + kFlushBlock - 1) / kFlushBlock;
+    int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
+    launch_kernel(cg_flush_shifts_kernel, grid, kFlushBlock, L.s, L.pdl, n2, ring, x, p, pstride, st, window);
+    return 1;
+}
+
+int launch_cg_update_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
                               CgState *st, Launch L)
 {
     long blocks = (n2 + kBlock - 1) / kBlock;
     int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
-    launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, r, y, p, pstride, st);
+    launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, ring, y, p, pstride, st);
     return 1;
 }
 

@@ -39,14 +39,19 @@ __device__ __forceinline__ void cg_step_beta(CgState *st, double rho_new)
     const int n = st->nshift;
     const double rho = st->rho, rho_b = st->rho_b;
     const double beta = rho_new / rho;
+    const int slot = st->iter % st->defer;       // this is iteration st->iter + 1: slot (n - 1) % defer
     if (k < n) {
         const int a = st->active[k];
         s_act[k] = a;
+        st->hist_on[slot][k] = a;
         if (a) {
             const double z = st->zeta[k], zn = st->zeta_new[k];
             const double ratio = zn / z;
             st->coef_z[k] = zn;
             st->coef_b[k] = beta * ratio * ratio;
+            st->hist_a[slot][k] = st->coef_a[k];     // written by this thread in cg_step_alpha
+            st->hist_z[slot][k] = zn;
+            st->hist_b[slot][k] = beta * ratio * ratio;
             st->zeta_old[k] = z;
             st->zeta[k] = zn;
             if (k > 0 && fabs(zn) * sqrt(rho_new) <= st->freeze * st->tol * sqrt(rho_b))

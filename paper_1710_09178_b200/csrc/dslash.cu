@@ -35,7 +35,7 @@ constexpr int kBlock = kDslashBlock;
 //            the seam sign of the backward hop is s-_mu(x).
 // WT = double2: the links as stored (p.W).  WT = float2: the fp32 copy p.W32 (NEXT-3, inner operator of
 // the mixed-precision solver, three rows only); every entry is widened on load, the arithmetic is fp64.
-template <bool XPAY, bool DOT, int ROWS, class WT = double2>
+template <bool XPAY, bool DOT, int ROWS, class WT = double2, bool KEEP = false>
 __global__ void __launch_bounds__(kBlock, ROWS == 2 ? QCD_DSLASH2_MINB : QCD_DSLASH3_MINB)
 dslash_kernel(const Geom g, const DslashParams p)
 {
@@ -59,8 +59,8 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
         for (int k = 0; k < NPF; ++k) {
             const int mu = k >> 1;
-            if (k & 1) load_link<ROWS>(W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
-            else load_link<ROWS>(W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
+            if (k & 1) load_link<ROWS, KEEP>(W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
+            else load_link<ROWS, KEEP>(W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
         }
     };
     // Inside the CG, `done` was last written two or more kernels back (r-update), which has completed
@@ -86,7 +86,7 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
                     for (int i = 0; i < 9; ++i) u[i] = pre[2 * mu < NPF ? 2 * mu : 0][i];
                 } else {
-                    load_link<ROWS>(w, Vh, u);
+                    load_link<ROWS, KEEP>(w, Vh, u);
                 }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hp[mu]);
@@ -106,7 +106,7 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
                     for (int i = 0; i < 9; ++i) u[i] = pre[2 * mu + 1 < NPF ? 2 * mu + 1 : 0][i];
                 } else {
-                    load_link<ROWS>(w, Vh, u);
+                    load_link<ROWS, KEEP>(w, Vh, u);
                 }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hm[mu]);
@@ -150,30 +150,33 @@ dslash_kernel(const Geom g, const DslashParams p)
 int dslash_chunks(const Geom &g) { return (g.st + kBlock - 1) / kBlock; }
 int dslash_grid_blocks(const Geom &g) { return dslash_chunks(g) * g.nt_run; }
 
-int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
+namespace {
+
+template <int ROWS, class WT, bool KEEP>
+void launch_variant(const Geom &g, const DslashParams &p, Launch L)
 {
     const int blocks = dslash_grid_blocks(g);
+    if (p.src == nullptr)
+        launch_kernel_apw(dslash_kernel<false, false, ROWS, WT, KEEP>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+    else if (p.dot_mode == 0)
+        launch_kernel_apw(dslash_kernel<true, false, ROWS, WT, KEEP>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+    else
+        launch_kernel_apw(dslash_kernel<true, true, ROWS, WT, KEEP>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+}
+
+}  // namespace
+
+int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
+{
     if (p.links32) {
-        if (p.src == nullptr)
-            launch_kernel_apw(dslash_kernel<false, false, 3, float2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
-        else if (p.dot_mode == 0)
-            launch_kernel_apw(dslash_kernel<true, false, 3, float2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
-        else
-            launch_kernel_apw(dslash_kernel<true, true, 3, float2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        if (p.keep_links) launch_variant<3, float2, true>(g, p, L);
+        else launch_variant<3, float2, false>(g, p, L);
     } else if (p.link_rows == 2) {
-        if (p.src == nullptr)
-            launch_kernel_apw(dslash_kernel<false, false, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
-        else if (p.dot_mode == 0)
-            launch_kernel_apw(dslash_kernel<true, false, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
-        else
-            launch_kernel_apw(dslash_kernel<true, true, 2>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        if (p.keep_links) launch_variant<2, double2, true>(g, p, L);
+        else launch_variant<2, double2, false>(g, p, L);
     } else {
-        if (p.src == nullptr)
-            launch_kernel_apw(dslash_kernel<false, false, 3>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
-        else if (p.dot_mode == 0)
-            launch_kernel_apw(dslash_kernel<true, false, 3>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
-        else
-            launch_kernel_apw(dslash_kernel<true, true, 3>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        if (p.keep_links) launch_variant<3, double2, true>(g, p, L);
+        else launch_variant<3, double2, false>(g, p, L);
     }
     return 1;
 }

@@ -71,13 +71,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
     } while (!ok);
 }
 // links are used once per apply: evict-first in L2, as the __ldcs of the register-staged kernel
-#ifndef QCD_BULK_L2_POLICY
-#define QCD_BULK_L2_POLICY "evict_first"     // tuning aid: "evict_normal", "evict_last"
-#endif
-__device__ __forceinline__ uint64_t evict_first_policy()
+// links are used once per apply: evict-first in L2, as the __ldcs of the register-staged kernel; or the
+// ordinary policy when the field is walked in alternating directions (DslashParams::keep_links)
+__device__ __forceinline__ uint64_t link_policy(bool keep)
 {
     uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::" QCD_BULK_L2_POLICY ".b64 %0, 1.0;" : "=l"(pol));
+    if (keep) asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    else asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     return pol;
 }
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t pol)
@@ -139,7 +139,7 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
 
     // one hop of the producer: wait for the stage to be free, announce the bytes, issue NW bulk copies
     Issue is{blockIdx.x, 0, 0, 0};
-    const uint64_t pol = evict_first_policy();
+    const uint64_t pol = link_policy(p.keep_links != 0);
     auto issue_one = [&]() {
         uint32_t t, sl0;
         tile_origin(g, p.reverse ? ntiles - 1 - is.tile : is.tile, t, sl0);
@@ -229,7 +229,7 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
                     } else {
                         const double2 *__restrict__ w = p.W + ((long)((bwd ? 1 - par : par) * 4 + mu) * NW) * Vh + src;
 #pragma unroll
-                        for (int i = 0; i < NW; ++i) u[i] = QCD_LINK_LOAD(w + (long)i * Vh);
+                        for (int i = 0; i < NW; ++i) u[i] = p.keep_links ? __ldg(w + (long)i * Vh) : __ldcs(w + (long)i * Vh);
                     }
                 }
                 __syncwarp();

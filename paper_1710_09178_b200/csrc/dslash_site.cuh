@@ -135,18 +135,18 @@ __device__ __forceinline__ double2 widen(float2 v) { return make_double2((double
 
 // u[0 .. 3*ROWS) <- the stored entries of one link (plane stride Vh); ROWS == 2: rebuild row 2.
 // WT = double2, or float2 for the fp32 copy of the links (NEXT-3: the arithmetic stays fp64).
-template <int ROWS, class WT>
+// KEEP = false: streaming (evict-first) loads.  Every link is used once per apply, so on a gauge field
+//   much larger than L2 the links should not push the vectors out (the output of one Dslash is the
+//   gathered input of the next) nor cycle through L2 in LRU order.  Measured, us per apply at 32^3x8 /
+//   48^3x12 / 64^3x16: __ldg 22.9 / 120.7 / 379.3, __ldcs 21.1 / 117.8 / 376.3.
+// KEEP = true: ordinary read-only loads, for gauge fields of about the size of L2 walked in alternating
+//   directions (QCD_OPT_SWEEP_ALTERNATE): what the previous apply touched last is still there.
+//   Measured at 32^3x8: 20.6 (streaming, one direction) -> 18.1 us; two-row 14.8 -> 13.5.
+template <int ROWS, bool KEEP = false, class WT>
 __device__ __forceinline__ void load_link(const WT *__restrict__ w, int Vh, double2 *u)
 {
-    // Links are used exactly once per apply: load them with the streaming (evict-first) policy, so that
-    // L2 keeps the vectors (the output of one Dslash is the gathered input of the next) and does not
-    // cycle the whole gauge field through LRU.  Measured, us per apply at 32^3x8 / 48^3x12 / 64^3x16:
-    // __ldg 22.9 / 120.7 / 379.3, __ldcs 21.1 / 117.8 / 376.3 (two-row at 32^3x8: 16.4 -> 15.5).
-#ifndef QCD_LINK_LOAD
-#define QCD_LINK_LOAD __ldcs
-#endif
 #pragma unroll
-    for (int i = 0; i < 3 * ROWS; ++i) u[i] = widen(QCD_LINK_LOAD(w + (long)i * Vh));
+    for (int i = 0; i < 3 * ROWS; ++i) u[i] = widen(KEEP ? __ldg(w + (long)i * Vh) : __ldcs(w + (long)i * Vh));
     if (ROWS == 2) third_row(u);
 }
 

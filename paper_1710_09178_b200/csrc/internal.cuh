@@ -17,6 +17,7 @@
 namespace qcd {
 
 constexpr int kMaxShifts = QCD_MAX_SHIFTS;
+constexpr int kMaxDefer = 8;   // iterations whose updates of the shifts k >= 1 can be applied in one pass (blas.cu)
 
 // n / d for 0 <= n < 2^31 with one mulhi (d fixed at context creation).
 struct FastDiv {
@@ -63,6 +64,12 @@ struct CgState {
     double scratch;               // generic reduction result (norms for true residuals)
     int not_su3;                  // set by the two-row gauge ingest (layout.cu)
     double cy[kMaxShifts];        // y-only mode: residues c_k of eq. 8 in sorted-shift order
+    // deferred shift updates (blas.cu): the coefficients of the last `defer` iterations, slot (n - 1) % defer
+    // for iteration n = 1, 2, ..., written by the last block of that iteration's r-update
+    int defer;                    // 1 <= defer <= kMaxDefer; also the number of slots of the residual ring
+    int enq;                      // iterations enqueued so far, dead ones included (r-update, CTA 0)
+    double hist_a[kMaxDefer][kMaxShifts], hist_z[kMaxDefer][kMaxShifts], hist_b[kMaxDefer][kMaxShifts];
+    int hist_on[kMaxDefer][kMaxShifts];   // shift k took part in the iteration of this slot
 };
 
 // ---- programmatic dependent launch (PDL) ----
@@ -145,6 +152,7 @@ struct DslashParams {
     double2 *out;
     int out_parity;
     int reverse;               // 1: the CTAs walk the tiles in descending order (QCD_OPT_SWEEP_ALTERNATE)
+    int keep_links;            // 1: links loaded with the ordinary policy (kept in L2), 0: streaming (evict-first)
     // optional fused epilogue: out = coeff * src - D in     (src on out_parity); src == nullptr: out = D in
     const double2 *src;
     double coeff;              // used when coeff_from_state == 0
@@ -190,14 +198,20 @@ int blas_grid_blocks(long n2);
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
                    double *partial, CgState *st, Launch L);
 // loop_handle != 0: the kernel is a node of a WHILE conditional graph and sets its condition
+// The residual lives in a ring of st->defer vectors (stride n2): r after iteration n is slot (n - 1) % defer,
+// the initial residual b is slot defer - 1.
 // pap_partial[0 .. npap): the per-CTA partial sums of <p_0,q> the preceding Dslash wrote
-int launch_cg_update_r(long n2, double2 *r, const double2 *q, const double *pap_partial, int npap,
+int launch_cg_update_r(long n2, double2 *ring, const double2 *q, const double *pap_partial, int npap,
                        double *partial, CgState *st, unsigned long long loop_handle, Launch L);
-// y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept)
-int launch_cg_update_shifts_y(long n2, const double2 *r, double2 *y, double2 *p, long pstride,
+// y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept; defer == 1)
+int launch_cg_update_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
                               CgState *st, Launch L);
-int launch_cg_update_shifts(long n2, const double2 *r, double2 *x, double2 *p, long pstride,
-                            CgState *st, Launch L);
+// x_k += alpha_k p_k ; p_k = zeta_k r + beta_k p_k for the shifts of this iteration; base_only: shift 0 alone
+int launch_cg_update_shifts(long n2, const double2 *ring, double2 *x, double2 *p, long pstride,
+                            CgState *st, int base_only, Launch L);
+// the deferred updates of the shifts k >= 1 for the last `window` enqueued iterations, in one pass
+int launch_cg_flush_shifts(long n2, const double2 *ring, double2 *x, double2 *p, long pstride,
+                           const CgState *st, int window, Launch L);
 // y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
                    int nshift, double c0, const double2 *b, double2 *y, Launch L);

@@ -426,6 +426,43 @@ def test_multishift_cg_is_deterministic(torch, q):
     assert np.array_equal(o1["x"], o2["x"]) and np.array_equal(o1["y"], o2["y"])
 
 
+def test_deferred_shift_updates_do_not_change_a_single_bit(torch, q):
+    """QCD_OPT_CG_DEFER: x_k, p_k of the shifts k >= 1 are updated once per m iterations from the stored
+    coefficients and a ring of residuals.  Same operations per element in the same order: every m,
+    every way of enqueueing, the freezing of shifts inside a window, max_iter inside a window and the
+    zero source give the bits of m = 1; and m = 1 matches the oracle."""
+    cases = [li.make_config_inputs(2)[:5]]
+    dims, mass = (4, 4, 4, 4), 0.005                      # light mass: shifts freeze one after the other
+    cases.append((li.Config(0, dims, mass, "random", 0.0, 16, 1e-6, 4.0, "ones", 1e-10),
+                  li.make_links(dims, "random", 5), li.make_source(dims, 5, E),
+                  np.logspace(-6, np.log10(4.0), 16), np.linspace(0.5, 2.0, 16)))
+    for cfg, links, b, shifts, res in cases:
+        rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+        rig.ctx.set_option(q.QCD_OPT_CG_DEFER, 1)
+        ref = rig.solve(E, b, shifts, res, cfg.tol)
+        exact = rig.lat.solve_exact(cfg.mass, E, b, shifts, res, cfg.tol)
+        check_solve(rig, cfg, b, shifts, res, ref, exact)
+        cut_ref = rig.solve(E, b, shifts, res, cfg.tol, max_iter=13)
+        for m, graph, batch in [(8, 1, 8), (2, 1, 8), (3, 0, 8), (5, 1, 3), (8, 2, 8), (4, 0, 1), (7, 1, 16), (8, 0, 5), (3, 2, 8)]:
+            rig.ctx.set_option(q.QCD_OPT_CG_DEFER, m)
+            rig.ctx.set_option(q.QCD_OPT_CG_GRAPH, graph)
+            rig.ctx.set_option(q.QCD_OPT_CG_BATCH, batch)
+            out = rig.solve(E, b, shifts, res, cfg.tol)
+            assert out["status"] == 0 and out["iterations"] == ref["iterations"], (m, graph, batch)
+            assert np.array_equal(out["x"], ref["x"]) and np.array_equal(out["y"], ref["y"]), (m, graph, batch)
+            assert np.array_equal(out["true_res"], ref["true_res"])
+            cut = rig.solve(E, b, shifts, res, cfg.tol, max_iter=13)
+            assert cut["status"] == 4 and cut["iterations"] == 13 and np.array_equal(cut["x"], cut_ref["x"])
+            zero = rig.solve(E, np.zeros_like(b), shifts, res, cfg.tol)
+            assert zero["status"] == 0 and zero["iterations"] == 0 and not zero["x"].any()
+            no_x = rig.solve(E, b, shifts, res, cfg.tol, own_x=False)
+            assert np.array_equal(no_x["y"], ref["y"])
+        for bad in (0, 9):
+            with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+                rig.ctx.set_option(q.QCD_OPT_CG_DEFER, bad)
+        rig.ctx.close()
+
+
 def test_execution_options_do_not_change_a_single_bit(torch, q):
     """QCD_OPT_PDL / QCD_OPT_CG_GRAPH / QCD_OPT_CG_BATCH only change how work is enqueued."""
     cfg, links, b, shifts, res = li.make_config_inputs(2)
