@@ -133,13 +133,15 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     launches a persistent grid of n CTAs per SM that walk the tiles round-robin.
  *                     Dslash and M^dag M stay bit-identical; CG results change at rounding level only
  *                     (the <p,Ap> partial sums are added per CTA).
- *   QCD_OPT_SWEEP_ALTERNATE  (default 2 = auto) 1: Dslash launches whose OUTPUT parity is even walk the
- *                     lattice in descending order, the others in ascending order, and the links are
- *                     loaded with the ordinary instead of the streaming policy.  D_oe and D_eo read the
- *                     same links, and inside M^dag M and the CG they alternate, so every apply starts on
- *                     the links its predecessor touched last, which are still in L2.  0: one direction,
- *                     streaming loads.  2: on when the stored links are at most twice the size of L2
- *                     (decided at qcd_load_gauge).  Dslash and M^dag M stay bit-identical.
+ *   QCD_OPT_SWEEP_ALTERNATE  (default 1) 1: Dslash launches whose OUTPUT parity is even walk the lattice in
+ *                     descending order, the others in ascending order, and the last
+ *                     QCD_OPT_SWEEP_KEEP_MB of link data of every sweep are left in L2 with the ordinary
+ *                     priority while the rest streams (evict-first).  D_oe and D_eo read the same links,
+ *                     and inside M^dag M and the CG they alternate, so every apply starts on the links
+ *                     its predecessor touched last.  0: one direction, all links streaming (the better
+ *                     setting for an isolated apply behind a cold L2).  Dslash and M^dag M stay
+ *                     bit-identical.
+ *   QCD_OPT_SWEEP_KEEP_MB (default 48) see above; 0 <= value <= 4096.
  *   QCD_OPT_MIXED     (default 0) SURVEY 8(f) NEXT-3, the mixed-precision variant the paper sets aside
  *                     (PAPER.md:168).  With 1, the NEXT qcd_load_gauge also stores an fp32 copy of the
  *                     three-row links (+288 V bytes), and qcd_multishift_cg becomes: (1) the fp64
@@ -157,7 +159,7 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
        QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8,
        QCD_OPT_MIXED = 9, QCD_OPT_MIXED_SWITCH_EXP = 10, QCD_OPT_OPERATOR_LINKS32 = 11,
-       QCD_OPT_SWEEP_ALTERNATE = 12, QCD_OPT_CG_DEFER = 13 };
+       QCD_OPT_SWEEP_ALTERNATE = 12, QCD_OPT_CG_DEFER = 13, QCD_OPT_SWEEP_KEEP_MB = 14 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

@@ -68,10 +68,11 @@ struct qcd_ctx {
     bool opt_operator_links32 = false;  // qcd_dslash / qcd_mdagm apply the fp32-link operator
     bool use_links32 = false;           // transient: the launches being enqueued use W32
     double2 *mx_r = nullptr, *mx_e = nullptr;
-    int opt_sweep_alternate = 2;        // 0 off, 1 on, 2 auto (on when the links are at most twice the size of L2)
+    int opt_sweep_alternate = 1;        // 0 off, 1 (or 2) on
     bool sweep_on = false;              // decided at qcd_load_gauge: even-output Dslash launches walk the tiles
                                         // backwards and the links are loaded with the ordinary (keep) policy
     size_t l2_bytes = 0;
+    int opt_keep_mb = 48;               // QCD_OPT_SWEEP_KEEP_MB: link bytes at the end of a sweep left in L2 with ordinary priority
     int opt_dslash_kernel = 0;          // 0: register-staged links (dslash.cu); 1: bulk-copy staged (dslash_bulk.cu)
     int opt_dslash_persist = 0;         // bulk kernel: CTAs per SM of a persistent grid (0: one CTA per tile)
     // cached graph of one batch of CG iterations (valid for exactly the key below)
@@ -158,16 +159,25 @@ void setup_l2_window(qcd_ctx *c)
 
 // QCD_OPT_SWEEP_ALTERNATE.  D_oe and D_eo read the SAME links (each reads the forward links of its output
 // parity and the backward links of the other), and inside M^dag M, the CG and any power iteration they
-// alternate.  On a gauge field of about the size of L2, walking the lattice in ascending order for odd
-// outputs and in descending order for even outputs lets every apply start on the links its predecessor
-// touched last -- still in L2 if they were loaded with the ordinary policy -- where a one-directional
-// sweep over more than L2 holds finds nothing of itself (LRU).  Measured at 32^3x8 (151 MB of links,
-// 126 MB of L2): 20.6 -> 18.1 us per apply, two-row (100 MB) 14.8 -> 13.5, solve 7.19 -> 6.95 ms; at
-// 48^3x12 (764 MB) and 64^3x16 (2.4 GB) nothing to win, and the streaming policy is the better one there.
-void decide_sweep(qcd_ctx *c)
+// alternate.  Walking the lattice in ascending order for odd outputs and in descending order for even
+// outputs lets every apply START on the links its predecessor touched LAST.  Those are still in L2 if
+// they were loaded with the ordinary priority while the rest of the sweep streamed past them with
+// evict-first: the last QCD_OPT_SWEEP_KEEP_MB of link data of every sweep are loaded "keep", everything
+// before "streaming" (per-CTA createpolicy operand of the link loads, dslash.cu).  Measured on B200, us per
+// apply in back-to-back (D_oe, D_eo) pairs, one direction + all streaming -> alternating + 48 MB kept:
+// 32^3x8 20.5 -> 16.0 (two-row 14.8 -> 11.9), 48^3x12 117.5 -> 112, 64^3x16 372.9 -> 367-370; 12-shift
+// solve at 32^3x8 5.27 -> 4.81 ms.  Keeping everything (the ordinary policy on all links) gives 18.1 us at
+// 32^3x8 and nothing at the larger sizes; 15 MB gives 18.0, 30 MB 16.9, 60 MB 16.2, 90 MB 16.9.  An
+// isolated launch behind a flushed L2 pays for it: 29.1 -> 30.7 us at 32^3x8.
+void decide_sweep(qcd_ctx *c) { c->sweep_on = c->opt_sweep_alternate != 0; }
+
+// CTAs at the end of a sweep whose links stay in L2 with the ordinary priority: opt_keep_mb of link data
+// (a CTA reads 8 links of 128 sites)
+int keep_tiles(const qcd_ctx *c)
 {
-    const size_t link_bytes = (size_t)c->g.Vh * 2 * 4 * 3 * c->link_rows * sizeof(double2);
-    c->sweep_on = c->opt_sweep_alternate == 1 || (c->opt_sweep_alternate == 2 && link_bytes <= 2 * c->l2_bytes);
+    const long per_tile = 128L * 8 * 3 * c->link_rows * (long)sizeof(double2);
+    const long n = (long)c->opt_keep_mb * 1000000L / per_tile;
+    return (int)std::min<long>(n, dslash_grid_blocks(c->g));
 }
 
 bool bad_parity(int p) { return p != QCD_EVEN && p != QCD_ODD; }
@@ -223,6 +233,7 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     p.W32 = c->W32; p.links32 = c->use_links32 ? 1 : 0;
     p.reverse = c->sweep_on && out_parity == QCD_EVEN ? 1 : 0;
     p.keep_links = c->sweep_on ? 1 : 0;
+    p.keep_tiles = c->sweep_on ? keep_tiles(c) : 0;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->pap_partial;
@@ -450,6 +461,12 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         if (value < 1 || value > 1024) return fail(c, QCD_EINVAL, "qcd_set_option: batch must be in [1, 1024]");
         c->opt_cg_batch = (int)value;
         return QCD_OK;
+    case QCD_OPT_SWEEP_KEEP_MB:
+        if (value < 0 || value > 4096) return fail(c, QCD_EINVAL, "qcd_set_option: keep size must be in [0, 4096] MB");
+        c->opt_keep_mb = (int)value;
+        for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);
+        c->cg_cache.clear(); c->cg_exec = nullptr;
+        return QCD_OK;
     case QCD_OPT_CG_DEFER:
         if (value < 1 || value > kMaxDefer) return fail(c, QCD_EINVAL, "qcd_set_option: defer must be in [1, 8]");
         c->opt_cg_defer = (int)value;
@@ -593,6 +610,7 @@ qcd_status qcd_dslash_range(qcd_ctx *c, int out_parity, const double *d_in, doub
     p.out_parity = out_parity; p.src = (const double2 *)d_src; p.coeff = coeff;
     p.reverse = c->sweep_on && out_parity == QCD_EVEN ? 1 : 0;
     p.keep_links = c->sweep_on ? 1 : 0;
+    p.keep_tiles = c->sweep_on ? keep_tiles(c) : 0;
     if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(g, p, c->Ld());
     return check_launch(c, "qcd_dslash_range");

@@ -17,6 +17,9 @@ namespace qcd {
 namespace {
 
 constexpr int kBlock = kDslashBlock;
+#ifndef QCD_LINK_HINT
+#define QCD_LINK_HINT 1      // 1: link loads carry the L2 priority as an operand, chosen per CTA (keep_tiles)
+#endif
 #ifndef QCD_DSLASH3_MINB
 #define QCD_DSLASH3_MINB 4   // 128 registers: 24.4 / 120.5 / 393 us; unbounded (60 regs) 26.0 / 129 / 404; 1 (254 regs) 25.7 / 120.2 / 394
 #endif
@@ -45,6 +48,14 @@ dslash_kernel(const Geom g, const DslashParams p)
                                                                  : reinterpret_cast<const WT *>(p.W);
     Site site;
     locate_tile<ROWS == 2>(g, p.out_parity, p.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x, threadIdx.x, site);
+#if QCD_LINK_HINT
+    // the last keep_tiles CTAs of the sweep leave their links in L2 with the ordinary priority (the next
+    // apply, walking the other way, starts there); the others stream (evict-first)
+    const uint64_t pol = l2_policy(blockIdx.x + (unsigned)p.keep_tiles >= gridDim.x);
+#define QCD_LOAD_LINK(w, u) load_link_hint<ROWS>(w, Vh, u, pol)
+#else
+#define QCD_LOAD_LINK(w, u) load_link<ROWS, KEEP>(w, Vh, u)
+#endif
     const bool valid = site.valid;
     const uint32_t h = site.h;
     const int par = p.out_parity;
@@ -59,8 +70,8 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
         for (int k = 0; k < NPF; ++k) {
             const int mu = k >> 1;
-            if (k & 1) load_link<ROWS, KEEP>(W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], Vh, pre[k]);
-            else load_link<ROWS, KEEP>(W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, pre[k]);
+            if (k & 1) QCD_LOAD_LINK(W + ((long)((1 - par) * 4 + mu) * NW) * Vh + hm[mu], pre[k]);
+            else QCD_LOAD_LINK(W + ((long)(par * 4 + mu) * NW) * Vh + h, pre[k]);
         }
     };
     // Inside the CG, `done` was last written two or more kernels back (r-update), which has completed
@@ -86,7 +97,7 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
                     for (int i = 0; i < 9; ++i) u[i] = pre[2 * mu < NPF ? 2 * mu : 0][i];
                 } else {
-                    load_link<ROWS, KEEP>(w, Vh, u);
+                    QCD_LOAD_LINK(w, u);
                 }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hp[mu]);
@@ -106,7 +117,7 @@ dslash_kernel(const Geom g, const DslashParams p)
 #pragma unroll
                     for (int i = 0; i < 9; ++i) u[i] = pre[2 * mu + 1 < NPF ? 2 * mu + 1 : 0][i];
                 } else {
-                    load_link<ROWS, KEEP>(w, Vh, u);
+                    QCD_LOAD_LINK(w, u);
                 }
 #pragma unroll
                 for (int c = 0; c < 3; ++c) v[c] = __ldg(in + (long)c * Vh + hm[mu]);

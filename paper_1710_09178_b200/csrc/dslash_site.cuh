@@ -150,4 +150,33 @@ __device__ __forceinline__ void load_link(const WT *__restrict__ w, int Vh, doub
     if (ROWS == 2) third_row(u);
 }
 
+// The same with the L2 eviction priority as a run-time operand (one code path for both policies, chosen
+// per CTA): ld.global.nc, no L1 allocation (a link is used once), L2 priority from a createpolicy value.
+__device__ __forceinline__ uint64_t l2_policy(bool keep)
+{
+    uint64_t pol;
+    if (keep) asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
+    else asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ double2 ld_hint(const double2 *p, uint64_t pol)
+{
+    double2 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ float2 ld_hint(const float2 *p, uint64_t pol)
+{
+    float2 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.x), "=f"(v.y) : "l"(p), "l"(pol));
+    return v;
+}
+template <int ROWS, class WT>
+__device__ __forceinline__ void load_link_hint(const WT *__restrict__ w, int Vh, double2 *u, uint64_t pol)
+{
+#pragma unroll
+    for (int i = 0; i < 3 * ROWS; ++i) u[i] = widen(ld_hint(w + (long)i * Vh, pol));
+    if (ROWS == 2) third_row(u);
+}
+
 }  // namespace qcd

@@ -153,6 +153,7 @@ struct DslashParams {
     int out_parity;
     int reverse;               // 1: the CTAs walk the tiles in descending order (QCD_OPT_SWEEP_ALTERNATE)
     int keep_links;            // 1: links loaded with the ordinary policy (kept in L2), 0: streaming (evict-first)
+    int keep_tiles;            // (QCD_LINK_HINT builds) CTAs at the end of the sweep that keep their links in L2
     // optional fused epilogue: out = coeff * src - D in     (src on out_parity); src == nullptr: out = D in
     const double2 *src;
     double coeff;              // used when coeff_from_state == 0
