@@ -97,7 +97,9 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     move once per m iterations instead of once per iteration (96 V/m bytes per shift
  *                     and iteration instead of 96 V).  Every element sees the same operations in the
  *                     same order: results are bit-identical to value 1 (update every iteration).
- *                     1 <= value <= 8.  Not used by the y-only form and single-shift solves.
+ *                     1 <= value <= 8.  The y-only form defers in the same way (y and the p_k of the shifts
+ *                     k >= 1 once per m iterations; y then agrees with value 1 to rounding, the sum being
+ *                     taken in another order).  Not used by single-shift solves.
  *   QCD_OPT_TGROUP    (default 0 = chosen by the library) order in which the Dslash CTAs walk the
  *                     lattice: groups of this many 128-site chunks of a t-slice are processed for all t
  *                     before the next group starts, so +-t neighbours are reused out of L2.  Dslash and

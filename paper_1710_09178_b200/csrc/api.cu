@@ -232,7 +232,6 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     p.W = c->W; p.link_rows = c->link_rows; p.in = in; p.out = out; p.out_parity = out_parity;
     p.W32 = c->W32; p.links32 = c->use_links32 ? 1 : 0;
     p.reverse = c->sweep_on && out_parity == QCD_EVEN ? 1 : 0;
-    p.keep_links = c->sweep_on ? 1 : 0;
     p.keep_tiles = c->sweep_on ? keep_tiles(c) : 0;
     p.src = src; p.coeff = coeff; p.coeff_from_state = coeff_from_state ? 1 : 0;
     p.mass2 = c->mass * c->mass;
@@ -255,15 +254,16 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
                                                : dslash_grid_blocks(c->g);
     c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, c->st, c->loop_handle, c->L());
     if (y_only)      // `x` is the single vector y
-        c->launches += launch_cg_update_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, c->L());
+        c->launches += launch_cg_update_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, c->cur_defer > 1 ? 1 : 0, c->L());
     else
         c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->cur_defer > 1 ? 1 : 0, c->L());
 }
 
 // the deferred updates of the shifts k >= 1 for the last `window` enqueued iterations
-void enqueue_cg_flush(qcd_ctx *c, double2 *x, int window)
+void enqueue_cg_flush(qcd_ctx *c, double2 *x, bool y_only, int window)
 {
-    c->launches += launch_cg_flush_shifts(c->n2, c->r, x, c->p, c->n2, c->st, window, c->L());
+    if (y_only) c->launches += launch_cg_flush_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, window, c->L());
+    else c->launches += launch_cg_flush_shifts(c->n2, c->r, x, c->p, c->n2, c->st, window, c->L());
 }
 
 // `count` iterations with the flushes that belong to them (count is a multiple of cur_defer, or the tail
@@ -273,7 +273,7 @@ void enqueue_cg_iterations(qcd_ctx *c, int parity, double2 *x, bool y_only, int 
     const int m = c->cur_defer;
     for (int i = 1; i <= count; ++i) {
         enqueue_cg_iteration(c, parity, x, y_only);
-        if (m > 1 && (i % m == 0 || i == count)) enqueue_cg_flush(c, x, i % m == 0 ? m : i % m);
+        if (m > 1 && (i % m == 0 || i == count)) enqueue_cg_flush(c, x, y_only, i % m == 0 ? m : i % m);
     }
 }
 
@@ -609,7 +609,6 @@ qcd_status qcd_dslash_range(qcd_ctx *c, int out_parity, const double *d_in, doub
     p.W = c->W; p.link_rows = c->link_rows; p.in = (const double2 *)d_in; p.out = (double2 *)d_out;
     p.out_parity = out_parity; p.src = (const double2 *)d_src; p.coeff = coeff;
     p.reverse = c->sweep_on && out_parity == QCD_EVEN ? 1 : 0;
-    p.keep_links = c->sweep_on ? 1 : 0;
     p.keep_tiles = c->sweep_on ? keep_tiles(c) : 0;
     if (c->opt_dslash_kernel == 1) c->launches += launch_dslash_bulk(g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(g, p, c->Ld());
@@ -682,9 +681,8 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     h.alpha_old = 1.0; h.beta_old = 0.0;
     h.tol = tol; h.freeze = 0.1;
     h.nshift = nshift; h.max_iter = max_iter;
-    // deferred updates of the shifts k >= 1 (blas.cu): not for the y-only form (it keeps no x_k) and
-    // pointless for a single shift
-    const int defer = (y_only || nshift == 1) ? 1 : std::max(1, std::min(c->opt_cg_defer, kMaxDefer));
+    // deferred updates of the shifts k >= 1 (blas.cu); pointless for a single shift
+    const int defer = nshift == 1 ? 1 : std::max(1, std::min(c->opt_cg_defer, kMaxDefer));
     h.defer = defer;
     c->cur_defer = defer;
     std::vector<long long> xoff_caller(nshift);

@@ -274,7 +274,7 @@ cg_flush_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__res
 // instead of x_k and p_k (96 V bytes); r and y once per element.
 __global__ void __launch_bounds__(kBlock)
 cg_update_shifts_y_kernel(long n2, const double2 *__restrict__ ring, double2 *__restrict__ y,
-                          double2 *__restrict__ p, long pstride, const CgState *__restrict__ st)
+                          double2 *__restrict__ p, long pstride, const CgState *__restrict__ st, int base_only)
 {
     pdl_wait();
     pdl_launch_dependents();
@@ -282,9 +282,9 @@ cg_update_shifts_y_kernel(long n2, const double2 *__restrict__ ring, double2 *__
     const double2 *__restrict__ r = ring + (long)((st->iter - 1) % st->defer) * n2;
     __shared__ double s_ca[kMaxShifts], s_z[kMaxShifts], s_b[kMaxShifts];
     __shared__ long long s_p[kMaxShifts];
-    const int nl = st->nlist;
+    const int nl = base_only ? 1 : st->nlist;       // base_only: the shifts k >= 1 are updated by the flush kernel
     if (threadIdx.x < nl) {
-        const int k = st->list[threadIdx.x];
+        const int k = base_only ? 0 : st->list[threadIdx.x];
         s_ca[threadIdx.x] = st->cy[k] * st->coef_a[k];
         s_z[threadIdx.x] = st->coef_z[k];
         s_b[threadIdx.x] = st->coef_b[k];
@@ -317,6 +317,100 @@ cg_update_shifts_y_kernel(long n2, const double2 *__restrict__ ring, double2 *__
             va.x = fma(s_b[j], va.x, s_z[j] * rv.x);
             va.y = fma(s_b[j], va.y, s_z[j] * rv.y);
             *pa = va;
+        }
+        y[i] = yv;
+    }
+}
+
+// Deferred form of the y-only update: y += sum_{k>=1} sum_n c_k alpha_k^(n) p_k^(n) and the p_k recurrences of
+// the last `window` iterations in one pass (see cg_flush_shifts_kernel): p_k of the shifts k >= 1 moves
+// once per defer iterations, y and the ring of residuals once per flush.
+__global__ void __launch_bounds__(kFlushBlock)
+cg_flush_shifts_y_kernel(long n2, const double2 *__restrict__ ring, double2 *__restrict__ y,
+                         double2 *__restrict__ p, long pstride, const CgState *__restrict__ st, int window)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    const int m = st->defer;
+    const int lo = st->enq - window, hi = min(st->enq, st->iter);
+    const int cnt = hi - lo;
+    if (cnt <= 0) return;
+    __shared__ double s_ca[kMaxDefer][kMaxShifts], s_z[kMaxDefer][kMaxShifts], s_b[kMaxDefer][kMaxShifts];
+    __shared__ long long s_p[kMaxShifts];
+    __shared__ int s_steps[kMaxShifts], s_all[kMaxShifts], s_map[kMaxShifts];
+    __shared__ int s_n;
+    const int ns = st->nshift;
+    if (threadIdx.x < kMaxShifts) {
+        const int k = threadIdx.x;
+        int steps = 0;
+        if (k >= 1 && k < ns)
+            while (steps < cnt && st->hist_on[(lo + steps) % m][k]) ++steps;
+        s_all[k] = steps;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int nl = 0;
+        for (int k = 1; k < ns; ++k)
+            if (s_all[k] > 0) {
+                s_map[nl] = k;
+                s_steps[nl] = s_all[k];
+                s_p[nl] = (long long)k * pstride;
+                ++nl;
+            }
+        s_n = nl;
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < cnt * s_n; idx += kFlushBlock) {
+        const int j = idx / s_n, l = idx - j * s_n, k = s_map[l], slot = (lo + j) % m;
+        s_ca[j][l] = st->cy[k] * st->hist_a[slot][k];
+        s_z[j][l] = st->hist_z[slot][k];
+        s_b[j][l] = st->hist_b[slot][k];
+    }
+    __syncthreads();
+    const int nl = s_n;
+    if (nl == 0) return;
+    for (long i = (long)blockIdx.x * kFlushBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kFlushBlock) {
+        double2 rv[kMaxDefer];
+#pragma unroll
+        for (int j = 0; j < kMaxDefer; ++j)
+            if (j < cnt) rv[j] = __ldg(ring + (long)((lo + j) % m) * n2 + i);
+        double2 yv = y[i];
+        int l = 0;
+        for (; l + 1 < nl; l += 2) {                // two shifts in flight per thread
+            double2 *pa = p + s_p[l] + i, *pb = p + s_p[l + 1] + i;
+            double2 pva = *pa, pvb = *pb;
+            const int sa = s_steps[l], sb = s_steps[l + 1];
+#pragma unroll
+            for (int j = 0; j < kMaxDefer; ++j) {
+                if (j < sa) {
+                    yv.x = fma(s_ca[j][l], pva.x, yv.x);
+                    yv.y = fma(s_ca[j][l], pva.y, yv.y);
+                    pva.x = fma(s_b[j][l], pva.x, s_z[j][l] * rv[j].x);
+                    pva.y = fma(s_b[j][l], pva.y, s_z[j][l] * rv[j].y);
+                }
+                if (j < sb) {
+                    yv.x = fma(s_ca[j][l + 1], pvb.x, yv.x);
+                    yv.y = fma(s_ca[j][l + 1], pvb.y, yv.y);
+                    pvb.x = fma(s_b[j][l + 1], pvb.x, s_z[j][l + 1] * rv[j].x);
+                    pvb.y = fma(s_b[j][l + 1], pvb.y, s_z[j][l + 1] * rv[j].y);
+                }
+            }
+            *pa = pva; *pb = pvb;
+        }
+        if (l < nl) {
+            double2 *pa = p + s_p[l] + i;
+            double2 pva = *pa;
+            const int sa = s_steps[l];
+#pragma unroll
+            for (int j = 0; j < kMaxDefer; ++j) {
+                if (j < sa) {
+                    yv.x = fma(s_ca[j][l], pva.x, yv.x);
+                    yv.y = fma(s_ca[j][l], pva.y, yv.y);
+                    pva.x = fma(s_b[j][l], pva.x, s_z[j][l] * rv[j].x);
+                    pva.y = fma(s_b[j][l], pva.y, s_z[j][l] * rv[j].y);
+                }
+            }
+            *pa = pva;
         }
         y[i] = yv;
     }
@@ -440,11 +534,20 @@ int launch_cg_flush_shifts(long n2, const double2 *ring, double2 *x, double2 *p,
 }
 
 int launch_cg_update_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
-                              CgState *st, Launch L)
+                              CgState *st, int base_only, Launch L)
 {
     long blocks = (n2 + kBlock - 1) / kBlock;
     int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
-    launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, ring, y, p, pstride, st);
+    launch_kernel(cg_update_shifts_y_kernel, grid, kBlock, L.s, L.pdl, n2, ring, y, p, pstride, st, base_only);
+    return 1;
+}
+
+int launch_cg_flush_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
+                             const CgState *st, int window, Launch L)
+{
+    long blocks = (n2 + kFlushBlock - 1) / kFlushBlock;
+    int grid = (int)(blocks < 148 * 8 ? (blocks > 0 ? blocks : 1) : 148 * 8);
+    launch_kernel(cg_flush_shifts_y_kernel, grid, kFlushBlock, L.s, L.pdl, n2, ring, y, p, pstride, st, window);
     return 1;
 }
 

@@ -17,9 +17,6 @@ namespace qcd {
 namespace {
 
 constexpr int kBlock = kDslashBlock;
-#ifndef QCD_LINK_HINT
-#define QCD_LINK_HINT 1      // 1: link loads carry the L2 priority as an operand, chosen per CTA (keep_tiles)
-#endif
 #ifndef QCD_DSLASH3_MINB
 #define QCD_DSLASH3_MINB 4   // 128 registers: 24.4 / 120.5 / 393 us; unbounded (60 regs) 26.0 / 129 / 404; 1 (254 regs) 25.7 / 120.2 / 394
 #endif
@@ -38,7 +35,7 @@ constexpr int kBlock = kDslashBlock;
 //            the seam sign of the backward hop is s-_mu(x).
 // WT = double2: the links as stored (p.W).  WT = float2: the fp32 copy p.W32 (NEXT-3, inner operator of
 // the mixed-precision solver, three rows only); every entry is widened on load, the arithmetic is fp64.
-template <bool XPAY, bool DOT, int ROWS, class WT = double2, bool KEEP = false>
+template <bool XPAY, bool DOT, int ROWS, class WT = double2>
 __global__ void __launch_bounds__(kBlock, ROWS == 2 ? QCD_DSLASH2_MINB : QCD_DSLASH3_MINB)
 dslash_kernel(const Geom g, const DslashParams p)
 {
@@ -48,14 +45,10 @@ dslash_kernel(const Geom g, const DslashParams p)
                                                                  : reinterpret_cast<const WT *>(p.W);
     Site site;
     locate_tile<ROWS == 2>(g, p.out_parity, p.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x, threadIdx.x, site);
-#if QCD_LINK_HINT
     // the last keep_tiles CTAs of the sweep leave their links in L2 with the ordinary priority (the next
-    // apply, walking the other way, starts there); the others stream (evict-first)
+    // apply, walking the other way, starts there); the others stream (evict-first): api.cu, decide_sweep
     const uint64_t pol = l2_policy(blockIdx.x + (unsigned)p.keep_tiles >= gridDim.x);
 #define QCD_LOAD_LINK(w, u) load_link_hint<ROWS>(w, Vh, u, pol)
-#else
-#define QCD_LOAD_LINK(w, u) load_link<ROWS, KEEP>(w, Vh, u)
-#endif
     const bool valid = site.valid;
     const uint32_t h = site.h;
     const int par = p.out_parity;
@@ -163,32 +156,25 @@ int dslash_grid_blocks(const Geom &g) { return dslash_chunks(g) * g.nt_run; }
 
 namespace {
 
-template <int ROWS, class WT, bool KEEP>
+template <int ROWS, class WT>
 void launch_variant(const Geom &g, const DslashParams &p, Launch L)
 {
     const int blocks = dslash_grid_blocks(g);
     if (p.src == nullptr)
-        launch_kernel_apw(dslash_kernel<false, false, ROWS, WT, KEEP>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        launch_kernel_apw(dslash_kernel<false, false, ROWS, WT>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
     else if (p.dot_mode == 0)
-        launch_kernel_apw(dslash_kernel<true, false, ROWS, WT, KEEP>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        launch_kernel_apw(dslash_kernel<true, false, ROWS, WT>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
     else
-        launch_kernel_apw(dslash_kernel<true, true, ROWS, WT, KEEP>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
+        launch_kernel_apw(dslash_kernel<true, true, ROWS, WT>, blocks, kBlock, L.s, L.pdl, L.apw, g, p);
 }
 
 }  // namespace
 
 int launch_dslash(const Geom &g, const DslashParams &p, Launch L)
 {
-    if (p.links32) {
-        if (p.keep_links) launch_variant<3, float2, true>(g, p, L);
-        else launch_variant<3, float2, false>(g, p, L);
-    } else if (p.link_rows == 2) {
-        if (p.keep_links) launch_variant<2, double2, true>(g, p, L);
-        else launch_variant<2, double2, false>(g, p, L);
-    } else {
-        if (p.keep_links) launch_variant<3, double2, true>(g, p, L);
-        else launch_variant<3, double2, false>(g, p, L);
-    }
+    if (p.links32) launch_variant<3, float2>(g, p, L);
+    else if (p.link_rows == 2) launch_variant<2, double2>(g, p, L);
+    else launch_variant<3, double2>(g, p, L);
     return 1;
 }
 

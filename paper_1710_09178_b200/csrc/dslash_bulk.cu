@@ -71,15 +71,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
     } while (!ok);
 }
 // links are used once per apply: evict-first in L2, as the __ldcs of the register-staged kernel
-// links are used once per apply: evict-first in L2, as the __ldcs of the register-staged kernel; or the
-// ordinary policy when the field is walked in alternating directions (DslashParams::keep_links)
-__device__ __forceinline__ uint64_t link_policy(bool keep)
-{
-    uint64_t pol;
-    if (keep) asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
-    else asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t pol)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
@@ -139,10 +130,12 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
 
     // one hop of the producer: wait for the stage to be free, announce the bytes, issue NW bulk copies
     Issue is{blockIdx.x, 0, 0, 0};
-    const uint64_t pol = link_policy(p.keep_links != 0);
+    // L2 priority of the link bytes, per tile as in dslash.cu: the last keep_tiles tiles of the sweep keep
+    const uint64_t pol_first = l2_policy(false), pol_keep = l2_policy(true);
     auto issue_one = [&]() {
         uint32_t t, sl0;
         tile_origin(g, p.reverse ? ntiles - 1 - is.tile : is.tile, t, sl0);
+        const uint64_t pol = is.tile + (uint32_t)p.keep_tiles >= ntiles ? pol_keep : pol_first;
         const int n = min(kTile, g.st - (int)sl0);
         const int h0 = (int)(t * (uint32_t)g.st + sl0);
         int lo, len;
@@ -187,6 +180,7 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
         uint32_t phase = 0;
         for (uint32_t seq = blockIdx.x; seq < ntiles; seq += gridDim.x) {
             const uint32_t tile = p.reverse ? ntiles - 1 - seq : seq;
+            const uint64_t pol = seq + (uint32_t)p.keep_tiles >= ntiles ? pol_keep : pol_first;
             Site site;
             locate_tile<ROWS == 2>(g, par, tile, threadIdx.x, site);
             const bool valid = site.valid;
@@ -229,7 +223,7 @@ dslash_bulk_kernel(const Geom g, const DslashParams p, const uint32_t ntiles)
                     } else {
                         const double2 *__restrict__ w = p.W + ((long)((bwd ? 1 - par : par) * 4 + mu) * NW) * Vh + src;
 #pragma unroll
-                        for (int i = 0; i < NW; ++i) u[i] = p.keep_links ? __ldg(w + (long)i * Vh) : __ldcs(w + (long)i * Vh);
+                        for (int i = 0; i < NW; ++i) u[i] = ld_hint(w + (long)i * Vh, pol);
                     }
                 }
                 __syncwarp();

@@ -134,24 +134,21 @@ __device__ __forceinline__ double2 widen(double2 v) { return v; }
 __device__ __forceinline__ double2 widen(float2 v) { return make_double2((double)v.x, (double)v.y); }
 
 // u[0 .. 3*ROWS) <- the stored entries of one link (plane stride Vh); ROWS == 2: rebuild row 2.
-// WT = double2, or float2 for the fp32 copy of the links (NEXT-3: the arithmetic stays fp64).
-// KEEP = false: streaming (evict-first) loads.  Every link is used once per apply, so on a gauge field
-//   much larger than L2 the links should not push the vectors out (the output of one Dslash is the
-//   gathered input of the next) nor cycle through L2 in LRU order.  Measured, us per apply at 32^3x8 /
-//   48^3x12 / 64^3x16: __ldg 22.9 / 120.7 / 379.3, __ldcs 21.1 / 117.8 / 376.3.
-// KEEP = true: ordinary read-only loads, for gauge fields of about the size of L2 walked in alternating
-//   directions (QCD_OPT_SWEEP_ALTERNATE): what the previous apply touched last is still there.
-//   Measured at 32^3x8: 20.6 (streaming, one direction) -> 18.1 us; two-row 14.8 -> 13.5.
-template <int ROWS, bool KEEP = false, class WT>
+// Streaming (evict-first) loads: every link is used once per apply, so the links should neither push the
+// vectors out of L2 (the output of one Dslash is the gathered input of the next) nor cycle through it in
+// LRU order.  Measured, us per apply at 32^3x8 / 48^3x12 / 64^3x16: __ldg 22.9 / 120.7 / 379.3, __ldcs
+// 21.1 / 117.8 / 376.3.
+template <int ROWS, class WT>
 __device__ __forceinline__ void load_link(const WT *__restrict__ w, int Vh, double2 *u)
 {
 #pragma unroll
-    for (int i = 0; i < 3 * ROWS; ++i) u[i] = widen(KEEP ? __ldg(w + (long)i * Vh) : __ldcs(w + (long)i * Vh));
+    for (int i = 0; i < 3 * ROWS; ++i) u[i] = widen(__ldcs(w + (long)i * Vh));
     if (ROWS == 2) third_row(u);
 }
 
 // The same with the L2 eviction priority as a run-time operand (one code path for both policies, chosen
-// per CTA): ld.global.nc, no L1 allocation (a link is used once), L2 priority from a createpolicy value.
+// per CTA; dslash.cu): ld.global.nc, no L1 allocation (a link is used once), L2 priority from a
+// createpolicy value -- evict_first reproduces the streaming load above (20.5 vs 20.6 us at 32^3x8).
 __device__ __forceinline__ uint64_t l2_policy(bool keep)
 {
     uint64_t pol;

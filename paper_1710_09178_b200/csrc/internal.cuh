@@ -152,8 +152,8 @@ struct DslashParams {
     double2 *out;
     int out_parity;
     int reverse;               // 1: the CTAs walk the tiles in descending order (QCD_OPT_SWEEP_ALTERNATE)
-    int keep_links;            // 1: links loaded with the ordinary policy (kept in L2), 0: streaming (evict-first)
-    int keep_tiles;            // (QCD_LINK_HINT builds) CTAs at the end of the sweep that keep their links in L2
+    int keep_tiles;            // tiles at the end of the sweep whose links stay in L2 with the ordinary priority
+                               // (all others are loaded evict-first)
     // optional fused epilogue: out = coeff * src - D in     (src on out_parity); src == nullptr: out = D in
     const double2 *src;
     double coeff;              // used when coeff_from_state == 0
@@ -204,9 +204,11 @@ int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstri
 // pap_partial[0 .. npap): the per-CTA partial sums of <p_0,q> the preceding Dslash wrote
 int launch_cg_update_r(long n2, double2 *ring, const double2 *q, const double *pap_partial, int npap,
                        double *partial, CgState *st, unsigned long long loop_handle, Launch L);
-// y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept; defer == 1)
+// y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept)
 int launch_cg_update_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
-                              CgState *st, Launch L);
+                              CgState *st, int base_only, Launch L);
+int launch_cg_flush_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
+                             const CgState *st, int window, Launch L);
 // x_k += alpha_k p_k ; p_k = zeta_k r + beta_k p_k for the shifts of this iteration; base_only: shift 0 alone
 int launch_cg_update_shifts(long n2, const double2 *ring, double2 *x, double2 *p, long pstride,
                             CgState *st, int base_only, Launch L);

@@ -926,6 +926,15 @@ def test_y_only_mode_gives_the_same_y_without_forming_x(torch, q, number, n):
         assert (tr1 <= 1.5 * tol).all() and (tr1 > 0).all()
         assert (tr0 <= 1.5 * tol).all()
         assert tr1[0] == pytest.approx(tr0[0], rel=0.05)          # base shift: recursion vs recomputed
+        # deferred (default, once per 8 iterations) against undeferred y-only accumulation: another order of
+        # the same sum
+        for m in (1, 3):
+            rig.ctx.set_option(q.QCD_OPT_CG_DEFER, m)
+            d_c = rig.ctx.new_vector()
+            st2, it2, tr2, _ = rig.ctx.apply_pow(E, d_phi, num, den, n, xmin, xmax, tol, 100000, d_c)
+            assert st2 == 0 and it2 == it1 and rel_l2(rig.to_canonical(E, d_c), yb) <= 1e-12
+            assert np.allclose(tr2, tr1, rtol=1e-9)
+        rig.ctx.set_option(q.QCD_OPT_CG_DEFER, 8)
     # the inv_sqrt entry point takes the same path; the zero source still works
     st, it, tr, _ = rig.ctx.inv_sqrt(E, torch.zeros_like(d_phi), n, xmin, xmax, tol, 100, d_b)
     assert st == 0 and it == 0 and not rig.to_canonical(E, d_b).any() and not tr.any()
