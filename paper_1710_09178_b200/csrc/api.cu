@@ -739,11 +739,14 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         DslashMultiParams mp{};
         mp.W = c->W; mp.link_rows = c->link_rows; mp.nrhs = nb;
         mp.partial = c->partial; mp.counter = &c->st->counter;
+        mp.keep_tiles = c->sweep_on ? keep_tiles(c) : 0;
         mp.out_parity = 1 - parity;                      // tmp_j = D_{q,p} x_j
+        mp.reverse = c->sweep_on && mp.out_parity == QCD_EVEN ? 1 : 0;
         mp.in = x; mp.out = c->p;
         for (int j = 0; j < nb; ++j) { mp.in_off[j] = h.xoff[k0 + j]; mp.out_off[j] = (long long)(k0 + j) * n2; }
         c->launches += launch_dslash_multi(c->g, mp, c->Ld());
         mp.out_parity = parity;                          // || b - ((m^2 + sigma_j) x_j - D_{p,q} tmp_j) ||^2
+        mp.reverse = c->sweep_on && mp.out_parity == QCD_EVEN ? 1 : 0;
         mp.in = c->p; mp.out = nullptr; mp.src = x; mp.b = b;
         for (int j = 0; j < nb; ++j) {
             mp.in_off[j] = (long long)(k0 + j) * n2;

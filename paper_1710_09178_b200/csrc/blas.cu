@@ -174,7 +174,14 @@ cg_update_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__re
 // the operations of the undeferred kernel in the same order: the results are bit-identical.
 // The kernel flushes the iterations (enq - window, min(enq, iter)]: enq counts the enqueued iterations
 // (dead ones included), iter the executed ones; neither is written while this kernel runs.
-constexpr int kFlushBlock = 256;
+#ifndef QCD_FLUSH_BLOCK
+#define QCD_FLUSH_BLOCK 256
+#endif
+#ifndef QCD_FLUSH_SHIFTS
+#define QCD_FLUSH_SHIFTS 2
+#endif
+constexpr int kFlushBlock = QCD_FLUSH_BLOCK;
+constexpr int kFlushShifts = QCD_FLUSH_SHIFTS;   // shifts whose x_k, p_k a thread has in flight at once
 
 __global__ void __launch_bounds__(kFlushBlock)
 cg_flush_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__restrict__ x,
@@ -227,42 +234,38 @@ cg_flush_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__res
 #pragma unroll
         for (int j = 0; j < kMaxDefer; ++j)
             if (j < cnt) rv[j] = __ldg(ring + (long)((lo + j) % m) * n2 + i);
-        int l = 0;
-        for (; l + 1 < nl; l += 2) {                // two shifts in flight per thread
-            double2 *xa = x + s_x[l] + i, *pa = p + s_p[l] + i, *xb = x + s_x[l + 1] + i, *pb = p + s_p[l + 1] + i;
-            double2 xva = *xa, pva = *pa, xvb = *xb, pvb = *pb;
-            const int sa = s_steps[l], sb = s_steps[l + 1];
+        for (int l = 0; l < nl; l += kFlushShifts) {       // kFlushShifts shifts in flight per thread
+            double2 xv[kFlushShifts], pv[kFlushShifts];
+            int steps[kFlushShifts];
 #pragma unroll
-            for (int j = 0; j < kMaxDefer; ++j) {
-                if (j < sa) {
-                    xva.x = fma(s_a[j][l], pva.x, xva.x);
-                    xva.y = fma(s_a[j][l], pva.y, xva.y);
-                    pva.x = fma(s_b[j][l], pva.x, s_z[j][l] * rv[j].x);
-                    pva.y = fma(s_b[j][l], pva.y, s_z[j][l] * rv[j].y);
-                }
-                if (j < sb) {
-                    xvb.x = fma(s_a[j][l + 1], pvb.x, xvb.x);
-                    xvb.y = fma(s_a[j][l + 1], pvb.y, xvb.y);
-                    pvb.x = fma(s_b[j][l + 1], pvb.x, s_z[j][l + 1] * rv[j].x);
-                    pvb.y = fma(s_b[j][l + 1], pvb.y, s_z[j][l + 1] * rv[j].y);
+            for (int s = 0; s < kFlushShifts; ++s) {
+                steps[s] = 0;
+                if (l + s < nl) {
+                    xv[s] = x[s_x[l + s] + i];
+                    pv[s] = p[s_p[l + s] + i];
+                    steps[s] = s_steps[l + s];
                 }
             }
-            *xa = xva; *pa = pva; *xb = xvb; *pb = pvb;
-        }
-        if (l < nl) {
-            double2 *xa = x + s_x[l] + i, *pa = p + s_p[l] + i;
-            double2 xva = *xa, pva = *pa;
-            const int sa = s_steps[l];
 #pragma unroll
             for (int j = 0; j < kMaxDefer; ++j) {
-                if (j < sa) {
-                    xva.x = fma(s_a[j][l], pva.x, xva.x);
-                    xva.y = fma(s_a[j][l], pva.y, xva.y);
-                    pva.x = fma(s_b[j][l], pva.x, s_z[j][l] * rv[j].x);
-                    pva.y = fma(s_b[j][l], pva.y, s_z[j][l] * rv[j].y);
+#pragma unroll
+                for (int s = 0; s < kFlushShifts; ++s) {
+                    if (j < steps[s]) {
+                        const double a = s_a[j][l + s], z = s_z[j][l + s], b = s_b[j][l + s];
+                        xv[s].x = fma(a, pv[s].x, xv[s].x);
+                        xv[s].y = fma(a, pv[s].y, xv[s].y);
+                        pv[s].x = fma(b, pv[s].x, z * rv[j].x);
+                        pv[s].y = fma(b, pv[s].y, z * rv[j].y);
+                    }
                 }
             }
-            *xa = xva; *pa = pva;
+#pragma unroll
+            for (int s = 0; s < kFlushShifts; ++s) {
+                if (l + s < nl) {
+                    x[s_x[l + s] + i] = xv[s];
+                    p[s_p[l + s] + i] = pv[s];
+                }
+            }
         }
     }
 }

@@ -26,7 +26,9 @@ dslash_multi_kernel(const Geom g, const DslashMultiParams p)
     const int Vh = g.Vh;
     const int par = p.out_parity;
     Site s;
-    locate<ROWS == 2>(g, par, s);
+    locate_tile<ROWS == 2>(g, par, p.reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x, threadIdx.x, s);
+    // alternating sweeps with the tail kept in L2, as in dslash.cu (the two launches of a batch have opposite parity)
+    const uint64_t pol = l2_policy(blockIdx.x + (unsigned)p.keep_tiles >= gridDim.x);
     pdl_wait();
     pdl_launch_dependents();
     double sum[NR];
@@ -41,7 +43,7 @@ dslash_multi_kernel(const Geom g, const DslashMultiParams p)
         for (int mu = 0; mu < 4; ++mu) {
             {   // forward hop
                 double2 u[9];
-                load_link<ROWS>(p.W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, u);
+                load_link_hint<ROWS>(p.W + ((long)(par * 4 + mu) * NW) * Vh + h, Vh, u, pol);
 #pragma unroll
                 for (int j = 0; j < NR; ++j) {
                     if (j < p.nrhs) {
@@ -61,7 +63,7 @@ dslash_multi_kernel(const Geom g, const DslashMultiParams p)
             }
             {   // backward hop
                 double2 u[9];
-                load_link<ROWS>(p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + s.hm[mu], Vh, u);
+                load_link_hint<ROWS>(p.W + ((long)((1 - par) * 4 + mu) * NW) * Vh + s.hm[mu], Vh, u, pol);
 #pragma unroll
                 for (int j = 0; j < NR; ++j) {
                     if (j < p.nrhs) {

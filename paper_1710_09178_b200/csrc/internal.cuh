@@ -180,6 +180,7 @@ constexpr int kMultiRhs = 4;
 struct DslashMultiParams {
     const double2 *W;
     int link_rows, out_parity, nrhs;
+    int reverse, keep_tiles;   // as in DslashParams
     const double2 *in;
     long long in_off[kMultiRhs];
     double2 *out;
