@@ -72,18 +72,21 @@ cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
     const int m = st->defer, it = st->iter;
     const double2 *rin = ring + (long)((it + m - 1) % m) * n2;     // == r when defer == 1: no __restrict__
     double2 *r = ring + (long)(it % m) * n2;
+    // the first chunk of r and q is requested BEFORE the alpha reduction: the loads do not depend on it and
+    // overlap its two barriers and its round trip to L2 (normally the only chunk: the grid covers the vector)
+    long base = (long)blockIdx.x * kRChunk + threadIdx.x;
+    double2 rv[kRUnroll], qv[kRUnroll];
+#pragma unroll
+    for (int e = 0; e < kRUnroll; ++e) {
+        const long i = base + (long)e * kBlock;
+        if (i < n2) { rv[e] = rin[i]; qv[e] = __ldg(q + i); }
+    }
     double t = 0.0;
     for (int i = threadIdx.x; i < npap; i += kBlock) t += __ldcg(pap_partial + i);
     const double pAp = block_sum<kBlock>(t);
     const double alpha = st->rho / pAp;   // st->rho is rewritten by the last block only, after every CTA has read it
     double s = 0.0;
-    for (long base = (long)blockIdx.x * kRChunk + threadIdx.x; base < n2; base += (long)gridDim.x * kRChunk) {
-        double2 rv[kRUnroll], qv[kRUnroll];
-#pragma unroll
-        for (int e = 0; e < kRUnroll; ++e) {
-            const long i = base + (long)e * kBlock;
-            if (i < n2) { rv[e] = rin[i]; qv[e] = __ldg(q + i); }
-        }
+    while (base < n2) {
 #pragma unroll
         for (int e = 0; e < kRUnroll; ++e) {
             const long i = base + (long)e * kBlock;
@@ -93,6 +96,12 @@ cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
                 r[i] = rv[e];
                 s += rv[e].x * rv[e].x + rv[e].y * rv[e].y;
             }
+        }
+        base += (long)gridDim.x * kRChunk;
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) { rv[e] = rin[i]; qv[e] = __ldg(q + i); }
         }
     }
     double total;
