@@ -100,6 +100,10 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     1 <= value <= 8.  The y-only form defers in the same way (y and the p_k of the shifts
  *                     k >= 1 once per m iterations; y then agrees with value 1 to rounding, the sum being
  *                     taken in another order).  Not used by single-shift solves.
+ *   QCD_OPT_CG_FUSE   (default 1) 1: the r-update and the base-shift update of an iteration run as ONE cooperative
+ *                     kernel with a grid-wide barrier between them (needs QCD_OPT_CG_DEFER > 1, not used
+ *                     by the y-only form and by QCD_OPT_CG_GRAPH = 2); 0: two kernels, the second
+ *                     waiting for the first's last block.  Bit-identical results.
  *   QCD_OPT_TGROUP    (default 0 = chosen by the library) order in which the Dslash CTAs walk the
  *                     lattice: groups of this many 128-site chunks of a t-slice are processed for all t
  *                     before the next group starts, so +-t neighbours are reused out of L2.  Dslash and
@@ -161,7 +165,7 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
 enum { QCD_OPT_PDL = 0, QCD_OPT_CG_GRAPH = 1, QCD_OPT_CG_BATCH = 2, QCD_OPT_LINK_ROWS = 3, QCD_OPT_TGROUP = 4,
        QCD_OPT_L2_PERSIST_MB = 5, QCD_OPT_Y_ONLY = 6, QCD_OPT_DSLASH_KERNEL = 7, QCD_OPT_DSLASH_PERSIST = 8,
        QCD_OPT_MIXED = 9, QCD_OPT_MIXED_SWITCH_EXP = 10, QCD_OPT_OPERATOR_LINKS32 = 11,
-       QCD_OPT_SWEEP_ALTERNATE = 12, QCD_OPT_CG_DEFER = 13, QCD_OPT_SWEEP_KEEP_MB = 14 };
+       QCD_OPT_SWEEP_ALTERNATE = 12, QCD_OPT_CG_DEFER = 13, QCD_OPT_SWEEP_KEEP_MB = 14, QCD_OPT_CG_FUSE = 15 };
 QCD_API qcd_status qcd_set_option(qcd_ctx *ctx, int option, long value);
 
 /* Size in doubles of one internal parity vector: 6 * V/2. */

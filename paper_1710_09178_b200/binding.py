@@ -17,7 +17,7 @@ import numpy as np
 QCD_EVEN, QCD_ODD = 0, 1
 QCD_OPT_PDL, QCD_OPT_CG_GRAPH, QCD_OPT_CG_BATCH, QCD_OPT_LINK_ROWS, QCD_OPT_TGROUP = 0, 1, 2, 3, 4
 QCD_OPT_L2_PERSIST_MB, QCD_OPT_Y_ONLY, QCD_OPT_DSLASH_KERNEL, QCD_OPT_DSLASH_PERSIST = 5, 6, 7, 8
-QCD_OPT_MIXED, QCD_OPT_MIXED_SWITCH_EXP, QCD_OPT_OPERATOR_LINKS32, QCD_OPT_SWEEP_ALTERNATE, QCD_OPT_CG_DEFER, QCD_OPT_SWEEP_KEEP_MB = 9, 10, 11, 12, 13, 14
+QCD_OPT_MIXED, QCD_OPT_MIXED_SWITCH_EXP, QCD_OPT_OPERATOR_LINKS32, QCD_OPT_SWEEP_ALTERNATE, QCD_OPT_CG_DEFER, QCD_OPT_SWEEP_KEEP_MB, QCD_OPT_CG_FUSE = 9, 10, 11, 12, 13, 14, 15
 QCD_OK, QCD_EINVAL, QCD_ENOMEM, QCD_ECUDA, QCD_ENOTCONV, QCD_ESTATE = range(6)
 _STATUS_NAMES = ["QCD_OK", "QCD_EINVAL", "QCD_ENOMEM", "QCD_ECUDA", "QCD_ENOTCONV", "QCD_ESTATE"]
 

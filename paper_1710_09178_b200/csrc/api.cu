@@ -57,6 +57,7 @@ struct qcd_ctx {
     unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
     bool opt_y_only = false;            // qcd_inv_sqrt / qcd_apply_pow accumulate y directly, no x_k
     int opt_cg_batch = 8;               // iterations enqueued per batch / per graph (rounded up to a multiple of defer)
+    bool opt_cg_fuse = true;            // QCD_OPT_CG_FUSE: r-update + base-shift update as one cooperative kernel
     int opt_cg_defer = kMaxDefer;       // QCD_OPT_CG_DEFER: iterations per deferred update of the shifts k >= 1
     int cur_defer = 1;                  // the value the solve being enqueued uses (1 for y-only and single-shift solves)
     int r_slots = 0;                    // vectors allocated in the residual ring c->r
@@ -79,14 +80,15 @@ struct qcd_ctx {
     cudaGraphExec_t cg_exec = nullptr;  // the entry of cg_cache selected by the last ensure_cg_graph
     cudaStream_t cap_stream = nullptr;  // capture-only stream (never executes work)
     struct CgKey {
-        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0, defer = 0; bool pdl = false, apw = false, yonly = false, l32 = false; double mass = 0.0;
+        int parity = -1, batch = 0, rows = 0, kern = 0, persist = 0, defer = 0; bool fuse = false; bool pdl = false, apw = false, yonly = false, l32 = false; double mass = 0.0;
         const void *x = nullptr, *p = nullptr, *q = nullptr, *r = nullptr, *tmp = nullptr;
         bool operator==(const CgKey &o) const {
-            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && defer == o.defer && pdl == o.pdl && apw == o.apw && yonly == o.yonly && l32 == o.l32 && mass == o.mass &&
+            return parity == o.parity && batch == o.batch && rows == o.rows && kern == o.kern && persist == o.persist && defer == o.defer && fuse == o.fuse && pdl == o.pdl && apw == o.apw && yonly == o.yonly && l32 == o.l32 && mass == o.mass &&
                    x == o.x && p == o.p && q == o.q && r == o.r && tmp == o.tmp;
         }
     };
-    struct CgGraph { CgKey key; cudaGraphExec_t exec; };
+    struct CgGraph { CgKey key; cudaGraphExec_t exec; long launches; };   // launches: kernels one replay runs
+    long cg_exec_launches = 0;          // of the selected graph
     std::vector<CgGraph> cg_cache;      // a few graphs: the mixed-precision solve alternates between two
     // L2 persistence of part of the gauge field (set at qcd_load_gauge; apw_on == false: none)
     cudaAccessPolicyWindow apw{};
@@ -252,6 +254,11 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
     run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
     const int npap = c->opt_dslash_kernel == 1 && !c->use_links32 ? dslash_bulk_grid_blocks(c->g, c->opt_dslash_persist)
                                                : dslash_grid_blocks(c->g);
+    if (c->opt_cg_fuse && !y_only && c->cur_defer > 1 && c->loop_handle == 0) {
+        const int n = launch_cg_update_r_base(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, x, c->p, c->st, c->L());
+        c->launches += n;
+        if (n) return;
+    }
     c->launches += launch_cg_update_r(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, c->st, c->loop_handle, c->L());
     if (y_only)      // `x` is the single vector y
         c->launches += launch_cg_update_shifts_y(c->n2, c->r, x, c->p, c->n2, c->st, c->cur_defer > 1 ? 1 : 0, c->L());
@@ -282,10 +289,10 @@ void enqueue_cg_iterations(qcd_ctx *c, int parity, double2 *x, bool y_only, int 
 qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y_only)
 {
     qcd_ctx::CgKey key;
-    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.kern = c->opt_dslash_kernel; key.persist = c->opt_dslash_persist; key.defer = c->cur_defer; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
+    key.parity = parity; key.batch = batch; key.rows = c->link_rows; key.kern = c->opt_dslash_kernel; key.persist = c->opt_dslash_persist; key.defer = c->cur_defer; key.fuse = c->opt_cg_fuse; key.pdl = c->opt_pdl; key.apw = c->apw_on; key.yonly = y_only; key.mass = c->mass;
     key.x = x; key.p = c->p; key.q = c->q; key.r = c->r; key.tmp = c->tmp; key.l32 = c->use_links32;
     for (auto &e : c->cg_cache)
-        if (e.key == key) { c->cg_exec = e.exec; return QCD_OK; }
+        if (e.key == key) { c->cg_exec = e.exec; c->cg_exec_launches = e.launches; return QCD_OK; }
     c->cg_exec = nullptr;
     if (c->cg_cache.size() >= 4) { cudaGraphExecDestroy(c->cg_cache.front().exec); c->cg_cache.erase(c->cg_cache.begin()); }
     if (!c->cap_stream)
@@ -333,12 +340,13 @@ qcd_status ensure_cg_graph(qcd_ctx *c, int parity, double2 *x, int batch, bool y
         if (graph) cudaGraphDestroy(graph);
     }
     c->stream = user;
+    c->cg_exec_launches = c->launches - launches0;
     c->launches = launches0;          // capturing launches nothing
     if (e != cudaSuccess) {
         c->cg_exec = nullptr;
         return fail(c, QCD_ECUDA, std::string("CG graph capture: ") + cudaGetErrorString(e));
     }
-    c->cg_cache.push_back({key, c->cg_exec});
+    c->cg_cache.push_back({key, c->cg_exec, c->cg_exec_launches});
     return QCD_OK;
 }
 
@@ -467,6 +475,7 @@ qcd_status qcd_set_option(qcd_ctx *c, int option, long value)
         for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);
         c->cg_cache.clear(); c->cg_exec = nullptr;
         return QCD_OK;
+    case QCD_OPT_CG_FUSE: c->opt_cg_fuse = value != 0; return QCD_OK;
     case QCD_OPT_CG_DEFER:
         if (value < 1 || value > kMaxDefer) return fail(c, QCD_EINVAL, "qcd_set_option: defer must be in [1, 8]");
         c->opt_cg_defer = (int)value;
@@ -716,7 +725,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         const int nb = use_graph ? batch : std::min(batch, max_iter - enq);
         if (use_graph) {
             QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));
-            c->launches += 4L * batch + (defer > 1 ? (batch + defer - 1) / defer : 0);
+            c->launches += c->cg_exec_launches;
         } else {
             enqueue_cg_iterations(c, parity, x, y_only, nb);
         }
@@ -770,7 +779,7 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     *iterations = h.iter;
     if (c->opt_cg_graph == 2) {          // the loop body (defer iterations and their flush) ran ceil(iter/defer) times
         const long bodies = std::max((h.iter + defer - 1) / defer, 1);
-        c->launches += bodies * (4L * defer + (defer > 1 ? 1 : 0));
+        c->launches += bodies * c->cg_exec_launches;
     }
     const double rho_b = h.rho_b;
     for (int k = 0; k < nshift; ++k)

@@ -4,6 +4,10 @@
 // update streams x_k and p_k of every active shift in one pass over r ("the heaviest kernel which
 // updates three large arrays").  All coefficients are read from the device-resident
 // CgState; nothing returns to the host inside an iteration.
+#include <algorithm>
+
+#include <cooperative_groups.h>
+
 #include "cg_scalars.cuh"
 #include "reduce.cuh"
 
@@ -112,6 +116,89 @@ cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
         // device-side loop (QCD_OPT_CG_GRAPH = 2): this iteration's shift update still runs (it is part
         // of the loop body); the WHILE node then stops when the stop test above has set `done`
         if (LOOP && threadIdx.x == 0) cudaGraphSetConditional(loop, st->done ? 0u : 1u);
+    }
+}
+
+// r-update AND base-shift update in one cooperative kernel (QCD_OPT_CG_FUSE = 1; SURVEY 7 hard part 3: "a
+// cooperative persistent kernel with grid.sync() for the BLAS-1 half of the iteration").  Phase 1 is the
+// r-update above; after grid.sync() every CTA adds the per-CTA partial sums of ||r'||^2 itself (consumer
+// side, fixed order: same bits everywhere), forms beta, and updates x_0, p_0; CTA 0 then runs the scalar
+// recurrences for all shifts.  For the base shift zeta stays exactly 1 (delta_0 = 0 in the recurrence),
+// so alpha_0 = alpha, the r-coefficient is 1 and beta_0 = beta: bit-identical to the two-kernel path.
+// Saves a kernel boundary, the ticket and the serial last-block pass; needs the whole grid co-resident.
+__global__ void __launch_bounds__(kBlock)
+cg_update_r_base_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
+                        const double *__restrict__ pap_partial, int npap, double *partial,
+                        double2 *__restrict__ x, double2 *__restrict__ p, CgState *st)
+{
+    pdl_wait();
+    pdl_launch_dependents();
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    if (blockIdx.x == 0 && threadIdx.x == 0) st->enq += 1;
+    if (st->done) {                       // dead iteration (every CTA sees the same flag: it is written after the grid sync only)
+        if (blockIdx.x == 0 && threadIdx.x == 0) st->done_prev = 1;
+        return;
+    }
+    const int m = st->defer, it = st->iter;
+    const double rho = st->rho;
+    const double2 *rin = ring + (long)((it + m - 1) % m) * n2;
+    double2 *r = ring + (long)(it % m) * n2;
+    double2 *__restrict__ x0 = x + st->xoff[0];
+    double t = 0.0;
+    for (int i = threadIdx.x; i < npap; i += kBlock) t += __ldcg(pap_partial + i);
+    const double pAp = block_sum<kBlock>(t);
+    const double alpha = rho / pAp;
+    double s = 0.0;
+    for (long base = (long)blockIdx.x * kRChunk + threadIdx.x; base < n2; base += (long)gridDim.x * kRChunk) {
+        double2 rv[kRUnroll], qv[kRUnroll];
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) { rv[e] = rin[i]; qv[e] = __ldg(q + i); }
+        }
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) {
+                rv[e].x = fma(-alpha, qv[e].x, rv[e].x);
+                rv[e].y = fma(-alpha, qv[e].y, rv[e].y);
+                r[i] = rv[e];
+                s += rv[e].x * rv[e].x + rv[e].y * rv[e].y;
+            }
+        }
+    }
+    const double bsum = block_sum<kBlock>(s);
+    if (threadIdx.x == 0) partial[blockIdx.x] = bsum;
+    __threadfence();
+    grid.sync();
+    double u = 0.0;
+    for (unsigned i = threadIdx.x; i < gridDim.x; i += kBlock) u += __ldcg(partial + i);
+    const double rho_new = block_sum<kBlock>(u);
+    const double beta = rho_new / rho;
+    for (long base = (long)blockIdx.x * kRChunk + threadIdx.x; base < n2; base += (long)gridDim.x * kRChunk) {
+        double2 rv[kRUnroll], xv[kRUnroll], pv[kRUnroll];
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) { rv[e] = r[i]; xv[e] = x0[i]; pv[e] = p[i]; }
+        }
+#pragma unroll
+        for (int e = 0; e < kRUnroll; ++e) {
+            const long i = base + (long)e * kBlock;
+            if (i < n2) {
+                xv[e].x = fma(alpha, pv[e].x, xv[e].x);
+                xv[e].y = fma(alpha, pv[e].y, xv[e].y);
+                pv[e].x = fma(beta, pv[e].x, 1.0 * rv[e].x);
+                pv[e].y = fma(beta, pv[e].y, 1.0 * rv[e].y);
+                x0[i] = xv[e];
+                p[i] = pv[e];
+            }
+        }
+    }
+    if (blockIdx.x == 0) {                // the scalar recurrences of all shifts, history, freezing, stop test
+        cg_step_alpha(st, pAp);
+        __syncthreads();
+        cg_step_beta(st, rho_new);
     }
 }
 
@@ -523,6 +610,40 @@ int launch_cg_update_r(long n2, double2 *ring, const double2 *q, const double *p
     else
         launch_kernel(cg_update_r_kernel<false>, grid, kBlock, L.s, L.pdl, n2, ring, q, pap_partial, npap, partial, st,
                       (cudaGraphConditionalHandle)0);
+    return 1;
+}
+
+// 0 if the cooperative launch is not possible (grid would not be co-resident)
+int launch_cg_update_r_base(long n2, double2 *ring, const double2 *q, const double *pap_partial, int npap,
+                            double *partial, double2 *x, double2 *p, CgState *st, Launch L)
+{
+    static int max_blocks = -1;
+    if (max_blocks < 0) {
+        int per_sm = 0, dev = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cg_update_r_base_kernel, kBlock, 0) != cudaSuccess) per_sm = 0;
+        max_blocks = per_sm * sms;
+    }
+    if (max_blocks <= 0) return 0;
+    const int grid = std::min(cg_update_r_grid_blocks(n2), max_blocks);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)kBlock);
+    cfg.stream = L.s;
+    cudaLaunchAttribute attr[2];
+    unsigned na = 0;
+    attr[na].id = cudaLaunchAttributeCooperative;
+    attr[na].val.cooperative = 1;
+    ++na;
+    if (L.pdl) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = na;
+    cudaLaunchKernelEx(&cfg, cg_update_r_base_kernel, n2, ring, q, pap_partial, npap, partial, x, p, st);
     return 1;
 }
 

@@ -457,6 +457,20 @@ def test_deferred_shift_updates_do_not_change_a_single_bit(torch, q):
             assert zero["status"] == 0 and zero["iterations"] == 0 and not zero["x"].any()
             no_x = rig.solve(E, b, shifts, res, cfg.tol, own_x=False)
             assert np.array_equal(no_x["y"], ref["y"])
+        # QCD_OPT_CG_FUSE: r-update and base-shift update as one cooperative kernel, same bits
+        rig.ctx.set_option(q.QCD_OPT_CG_FUSE, 1)
+        for m, graph, batch in [(8, 1, 8), (4, 0, 8), (8, 2, 8), (3, 1, 5)]:
+            rig.ctx.set_option(q.QCD_OPT_CG_DEFER, m)
+            rig.ctx.set_option(q.QCD_OPT_CG_GRAPH, graph)
+            rig.ctx.set_option(q.QCD_OPT_CG_BATCH, batch)
+            out = rig.solve(E, b, shifts, res, cfg.tol)
+            assert out["status"] == 0 and out["iterations"] == ref["iterations"], (m, graph, batch)
+            assert np.array_equal(out["x"], ref["x"]) and np.array_equal(out["y"], ref["y"]), (m, graph, batch)
+            cut = rig.solve(E, b, shifts, res, cfg.tol, max_iter=13)
+            assert cut["status"] == 4 and cut["iterations"] == 13 and np.array_equal(cut["x"], cut_ref["x"])
+            zero = rig.solve(E, np.zeros_like(b), shifts, res, cfg.tol)
+            assert zero["status"] == 0 and zero["iterations"] == 0 and not zero["x"].any()
+        rig.ctx.set_option(q.QCD_OPT_CG_FUSE, 0)
         for bad in (0, 9):
             with pytest.raises(q.QcdError, match="QCD_EINVAL"):
                 rig.ctx.set_option(q.QCD_OPT_CG_DEFER, bad)
