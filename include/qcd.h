@@ -196,6 +196,27 @@ QCD_API qcd_status qcd_dslash(qcd_ctx *ctx, int out_parity, const double *d_in, 
 QCD_API qcd_status qcd_dslash_range(qcd_ctx *ctx, int out_parity, const double *d_in, double *d_out,
                                     int t0, int nt, const double *d_src, double coeff);
 
+/* Slab (distributed) mode, SURVEY 8(f) NEXT-4 (slabs with halos, a face
+ * exchange before every D, two reduced scalars per CG iteration).  With enable != 0 the context's lattice
+ * is ONE RANK'S t-slab held with one halo slice on either side (extents Nx, Ny, Nz, nt_owned + 2; see
+ * paper_1710_09178_b200/slab.py for the index maps, the parity flip and the seam carried by the links).
+ * From then on
+ *   qcd_dslash, qcd_mdagm      call halo(user, d_in, stream) first -- the caller fills the two halo t-slices
+ *                              of that internal vector, WHICH IS THEREFORE WRITTEN -- and compute the owned
+ *                              slices 1 .. Nt-2 only; the halo slices of the output are left untouched;
+ *   qcd_multishift_cg          additionally calls allreduce(user, d_buf, count, stream) wherever an inner
+ *                              product leaves the rank (||b||^2, <p_0,q> and ||r||^2 once per iteration,
+ *                              the residual norms at the end): an in-place SUM over the ranks of `count`
+ *                              doubles in DEVICE memory.  The halo slices of d_b are ignored (taken as
+ *                              zero); those of d_x and d_y hold no result.  Every rank
+ *                              runs the same iteration on replicated scalars, so all ranks make the same
+ *                              calls in the same order.  No CUDA graphs, no PDL in this mode.
+ * Both callbacks must be ordered on `stream` (they may synchronise it).  QCD_OPT_MIXED and the y-only form
+ * are not available in slab mode.  halo, allreduce: see the typedefs. */
+typedef void (*qcd_halo_fn)(void *user, double *d_vec, void *cuda_stream);
+typedef void (*qcd_allreduce_fn)(void *user, double *d_buf, int count, void *cuda_stream);
+QCD_API qcd_status qcd_set_slab(qcd_ctx *ctx, int enable, qcd_halo_fn halo, qcd_allreduce_fn allreduce, void *user);
+
 /* a4: d_out = m^2 d_in - D_{p,q} D_{q,p} d_in on `parity` p  (C3).
  * Internal layout; d_in and d_out must not alias. */
 QCD_API qcd_status qcd_mdagm(qcd_ctx *ctx, int parity, const double *d_in, double *d_out);

@@ -41,6 +41,7 @@ _SIGNATURES = {
     "qcd_unpack": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_dslash": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_dslash_range": (_ci, [_vp, _ci, _vp, _vp, _ci, _ci, _vp, _cd]),
+    "qcd_set_slab": (_ci, [_vp, _ci, _vp, _vp, _vp]),
     "qcd_mdagm": (_ci, [_vp, _ci, _vp, _vp]),
     "qcd_multishift_cg": (_ci, [_vp, _ci, _vp, _ci, _vp, _vp, _cd, _ci, _vp, _vp,
                                 ctypes.POINTER(_ci), _vp]),
@@ -173,6 +174,9 @@ class Context:
     __del__ = close
 
     def _check(self, st: int, where: str, allow=()):
+        exc, self._slab_exc = getattr(self, "_slab_exc", None), None
+        if exc is not None:
+            raise exc
         if st != QCD_OK and st not in allow:
             raise QcdError(st, where, self._lib.qcd_last_error(self._h).decode())
         return st
@@ -217,6 +221,30 @@ class Context:
         self._check(self._lib.qcd_dslash_range(self._h, out_parity, _dev_ptr(d_in, vd), _dev_ptr(d_out, vd),
                                                int(t0), int(nt), None if d_src is None else _dev_ptr(d_src, vd),
                                                float(coeff)), "qcd_dslash_range")
+
+    def set_slab(self, halo=None, allreduce=None):
+        """qcd_set_slab.  halo(ptr: int, stream: int) fills the two halo t-slices of the internal vector at
+        device address ptr; allreduce(ptr: int, count: int, stream: int) sums count doubles at device address
+        ptr over the ranks, in place.  Both None: leave slab mode.  The ctypes trampolines are kept alive here."""
+        if halo is None and allreduce is None:
+            self._slab_cbs = None
+            self._check(self._lib.qcd_set_slab(self._h, 0, None, None, None), "qcd_set_slab")
+            return
+        halo_t = ctypes.CFUNCTYPE(None, _vp, _vp, _vp)
+        red_t = ctypes.CFUNCTYPE(None, _vp, _vp, _ci, _vp)
+        self._slab_exc = None
+
+        def guard(fn, *a):          # an exception must not unwind through the C frames: keep it for _check
+            try:
+                fn(*a)
+            except BaseException as e:  # noqa: BLE001
+                if self._slab_exc is None:
+                    self._slab_exc = e
+
+        h = halo_t(lambda user, ptr, stream: guard(halo, int(ptr or 0), int(stream or 0)))
+        r = red_t(lambda user, ptr, count, stream: guard(allreduce, int(ptr or 0), int(count), int(stream or 0)))
+        self._slab_cbs = (h, r)
+        self._check(self._lib.qcd_set_slab(self._h, 1, ctypes.cast(h, _vp), ctypes.cast(r, _vp), None), "qcd_set_slab")
 
     def mdagm(self, parity: int, d_in, d_out):
         self._check(self._lib.qcd_mdagm(self._h, parity, _dev_ptr(d_in, self.vector_doubles), _dev_ptr(d_out, self.vector_doubles)), "qcd_mdagm")

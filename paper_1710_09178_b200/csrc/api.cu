@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstddef>
 #include <cstdint>
 #include <cstring>
 #include <new>
@@ -57,6 +58,12 @@ struct qcd_ctx {
     unsigned long long loop_handle = 0; // conditional handle while the body of the loop graph is captured
     bool opt_y_only = false;            // qcd_inv_sqrt / qcd_apply_pow accumulate y directly, no x_k
     int opt_cg_batch = 8;               // iterations enqueued per batch / per graph (rounded up to a multiple of defer)
+    // slab (distributed) mode: the lattice of this context is a t-slab with one halo slice
+    // on either side; halo fills and sums over the ranks are the caller's (qcd_set_slab)
+    bool slab = false;
+    qcd_halo_fn halo = nullptr;
+    qcd_allreduce_fn allreduce = nullptr;
+    void *slab_user = nullptr;
     bool opt_cg_fuse = true;            // QCD_OPT_CG_FUSE: r-update + base-shift update as one cooperative kernel
     int opt_cg_defer = kMaxDefer;       // QCD_OPT_CG_DEFER: iterations per deferred update of the shifts k >= 1
     int cur_defer = 1;                  // the value the solve being enqueued uses (1 for y-only and single-shift solves)
@@ -94,11 +101,11 @@ struct qcd_ctx {
     cudaAccessPolicyWindow apw{};
     bool apw_on = false;
     long opt_l2_persist_mb = 0;         // QCD_OPT_L2_PERSIST_MB
-    Launch L() const { return Launch{stream, opt_pdl, nullptr}; }
+    Launch L() const { return Launch{stream, opt_pdl && !slab, nullptr}; }
     // Dslash launches: they read links before their PDL wait, so the first one after a gauge load must
     // be fully serialised behind the ingest kernel
     bool fresh_gauge = false;
-    Launch Ld() { const bool pdl = opt_pdl && !fresh_gauge; fresh_gauge = false; return Launch{stream, pdl, apw_on ? &apw : nullptr}; }
+    Launch Ld() { const bool pdl = opt_pdl && !fresh_gauge && !slab; fresh_gauge = false; return Launch{stream, pdl, apw_on ? &apw : nullptr}; }
 };
 
 static std::string g_create_err;
@@ -203,7 +210,10 @@ qcd_status ensure_host_staging(qcd_ctx *c)
 
 qcd_status ensure_cg_workspace(qcd_ctx *c, int nshift, bool need_x)
 {
-    if (!c->q) QCD_CUDA(c, dev_alloc(&c->q, (size_t)c->n2));
+    if (!c->q) {
+        QCD_CUDA(c, dev_alloc(&c->q, (size_t)c->n2));
+        QCD_CUDA(c, cudaMemsetAsync(c->q, 0, c->vec_bytes, c->stream));   // slab mode: its halo slices are never written
+    }
     if (c->r_slots < kMaxDefer) {          // the residual ring (deferred shift updates, blas.cu)
         if (c->r) cudaFree(c->r);
         c->r = nullptr; c->r_slots = 0;
@@ -239,10 +249,22 @@ qcd_status run_dslash(qcd_ctx *c, int out_parity, const double2 *in, double2 *ou
     p.mass2 = c->mass * c->mass;
     p.dot_mode = dot_mode; p.partial = c->pap_partial;
     p.st = (gated || dot_mode || coeff_from_state) ? c->st : nullptr;
+    if (c->slab) {       // the caller fills the two halo slices of the input; the owned slices 1 .. Nt-2 are computed
+        c->halo(c->slab_user, (double *)in, (void *)c->stream);
+        Geom g = c->g;
+        g.t0 = 1; g.nt_run = g.Nt - 2;
+        p.keep_tiles = std::min(p.keep_tiles, dslash_grid_blocks(g));
+        c->launches += launch_dslash(g, p, c->Ld());
+        return QCD_OK;
+    }
     if (c->opt_dslash_kernel == 1 && !c->use_links32) c->launches += launch_dslash_bulk(c->g, p, c->opt_dslash_persist, c->Ld());
     else c->launches += launch_dslash(c->g, p, c->Ld());
     return QCD_OK;
 }
+
+// slab mode: sum `count` doubles of the device-resident state over the ranks (stream-ordered)
+void slab_allreduce(qcd_ctx *c, double *d_buf, int count) { c->allreduce(c->slab_user, d_buf, count, (void *)c->stream); }
+double *state_field(qcd_ctx *c, size_t offset) { return (double *)((char *)c->st + offset); }
 
 // one multishift-CG iteration: 4 kernels, all scalars stay on the device.  With deferred
 // shift updates (cur_defer > 1) the fourth kernel updates the base shift only; the caller enqueues
@@ -252,6 +274,18 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
     // tmp = D_{q,p} p_0 ; q = (m^2 + sigma_0) p_0 - D_{p,q} tmp, <p_0,q> -> alpha, zeta_new
     run_dslash(c, 1 - parity, c->p, c->tmp, nullptr, 0.0, false, 0, true);
     run_dslash(c, parity, c->tmp, c->q, c->p, 0.0, true, 1, true);
+    if (c->slab) {       // the two inner products leave the rank between the kernels (reading N4)
+        Geom g = c->g;
+        g.t0 = 1; g.nt_run = g.Nt - 2;
+        double *red = state_field(c, offsetof(CgState, red));
+        c->launches += launch_sum_partials(c->pap_partial, dslash_grid_blocks(g), red, c->L());
+        slab_allreduce(c, red, 1);                                   // <p_0,q>
+        c->launches += launch_cg_update_r_split(c->n2, c->r, c->q, red, c->partial, c->st, c->L());
+        slab_allreduce(c, red + 1, 1);                               // ||r'||^2
+        c->launches += launch_cg_scalars(c->st, c->L());
+        c->launches += launch_cg_update_shifts(c->n2, c->r, x, c->p, c->n2, c->st, c->cur_defer > 1 ? 1 : 0, c->L());
+        return;
+    }
     const int npap = c->opt_dslash_kernel == 1 && !c->use_links32 ? dslash_bulk_grid_blocks(c->g, c->opt_dslash_persist)
                                                : dslash_grid_blocks(c->g);
     if (c->opt_cg_fuse && !y_only && c->cur_defer > 1 && c->loop_handle == 0) {
@@ -602,6 +636,19 @@ qcd_status qcd_dslash(qcd_ctx *c, int out_parity, const double *d_in, double *d_
     return check_launch(c, "qcd_dslash");
 }
 
+qcd_status qcd_set_slab(qcd_ctx *c, int enable, qcd_halo_fn halo, qcd_allreduce_fn allreduce, void *user)
+{
+    if (!c) return QCD_EINVAL;
+    if (enable && (!halo || !allreduce)) return fail(c, QCD_EINVAL, "qcd_set_slab: both callbacks are needed");
+    if (enable && c->g.Nt < 4) return fail(c, QCD_EINVAL, "qcd_set_slab: a slab needs two halo slices and at least two owned ones");
+    c->slab = enable != 0;
+    c->halo = halo; c->allreduce = allreduce; c->slab_user = user;
+    if (c->slab && c->q) QCD_CUDA(c, cudaMemsetAsync(c->q, 0, c->vec_bytes, c->stream));   // its halo slices must be zero
+    for (auto &e : c->cg_cache) cudaGraphExecDestroy(e.exec);
+    c->cg_cache.clear(); c->cg_exec = nullptr;
+    return QCD_OK;
+}
+
 qcd_status qcd_dslash_range(qcd_ctx *c, int out_parity, const double *d_in, double *d_out, int t0, int nt,
                             const double *d_src, double coeff)
 {
@@ -670,6 +717,8 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
         return fail(c, QCD_EINVAL, "qcd_multishift_cg: d_b, d_x and d_y must not overlap");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_multishift_cg: no gauge field loaded");
     y_only = y_only && d_x == nullptr && d_y != nullptr;
+    if (c->slab && (y_only || c->use_links32))
+        return fail(c, QCD_EINVAL, "qcd_multishift_cg: slab mode supports the plain fp64 solver only");
     qcd_status s = ensure_cg_workspace(c, nshift, d_x == nullptr && !y_only);
     if (s != QCD_OK) return s;
 
@@ -707,12 +756,18 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
     QCD_CUDA(c, cudaMemcpyAsync(c->st, &h, sizeof h, cudaMemcpyHostToDevice, st));
     QCD_CUDA(c, cudaMemsetAsync(x, 0, (size_t)n2 * (y_only ? 1 : nshift) * sizeof(double2), st));
     // the initial residual b is slot defer - 1 of the ring: "r after iteration 0"
-    c->launches += launch_cg_init(n2, b, c->r + (long)(defer - 1) * n2, c->p, n2, nshift, c->partial, c->st, c->L());
+    c->launches += launch_cg_init(n2, b, c->r + (long)(defer - 1) * n2, c->p, n2, nshift, c->partial, c->st,
+                                  c->g.Vh, c->slab ? c->g.st : 0, c->L());
+
+    if (c->slab) {       // ||b||^2 over all ranks; a rank whose part of the source vanishes must still iterate
+        slab_allreduce(c, state_field(c, offsetof(CgState, rho)), 1);
+        c->launches += launch_cg_after_init(c->st, c->L());
+    }
 
     // iteration loop: enqueue only (one graph replay, or 4 launches per iteration, per batch)
     const int batch = std::max(1, std::min(c->opt_cg_batch, max_iter));
-    const bool use_graph = c->opt_cg_graph == 1;
-    if (c->opt_cg_graph == 2) {
+    const bool use_graph = c->opt_cg_graph == 1 && !c->slab;    // slab mode: the callbacks are not captured
+    if (c->opt_cg_graph == 2 && !c->slab) {
         if ((s = ensure_cg_graph(c, parity, x, 0, y_only)) != QCD_OK) return s;
         QCD_CUDA(c, cudaGraphLaunch(c->cg_exec, st));     // launch count added below, once iter is known
     } else {
@@ -743,7 +798,18 @@ qcd_status multishift_cg_impl(qcd_ctx *c, int parity, const double *d_b, int nsh
 
     // finish (a6): true residuals recomputed from x_k, kMultiRhs shifts per pass over the links;
     // the p_k are dead by now and serve as the tmp vectors.  y = sum_k c_k x_k.
-    for (int k0 = 0; k0 < (y_only || !finish ? 0 : nshift); k0 += kMultiRhs) {
+    if (c->slab && finish) {        // true residuals shift by shift: halo fills are per vector; norms summed over the ranks
+        if (!c->mx_r) QCD_CUDA(c, dev_alloc(&c->mx_r, (size_t)n2));
+        for (int k = 0; k < nshift; ++k) {
+            double2 *xk = x + h.xoff[k];
+            run_dslash(c, 1 - parity, xk, c->tmp, nullptr, 0.0, false, 0, false);
+            run_dslash(c, parity, c->tmp, c->q, xk, c->mass * c->mass + h.sigma[k], false, 0, false);
+            c->launches += launch_residual(n2, b, c->q, c->mx_r, c->partial, &c->st->counter, c->results + order[k],
+                                           c->g.Vh, c->g.st, c->L());
+        }
+        slab_allreduce(c, c->results, nshift);
+    }
+    for (int k0 = 0; k0 < (y_only || !finish || c->slab ? 0 : nshift); k0 += kMultiRhs) {
         const int nb = std::min(kMultiRhs, nshift - k0);
         DslashMultiParams mp{};
         mp.W = c->W; mp.link_rows = c->link_rows; mp.nrhs = nb;
@@ -830,7 +896,7 @@ qcd_status mixed_multishift_cg(qcd_ctx *c, int parity, const double *d_b, int ns
             // r = b - ((m^2 + sigma_k) x_k - D_{p,q} D_{q,p} x_k), fp64 links
             run_dslash(c, 1 - parity, xk, c->tmp, nullptr, 0.0, false, 0, false);
             run_dslash(c, parity, c->tmp, c->q, xk, coeff, false, 0, false);
-            c->launches += launch_residual(n2, b, c->q, c->mx_r, c->partial, &c->st->counter, c->results, c->L());
+            c->launches += launch_residual(n2, b, c->q, c->mx_r, c->partial, &c->st->counter, c->results, c->g.Vh, 0, c->L());
             if ((s = check_launch(c, "qcd_multishift_cg (mixed)")) != QCD_OK) return s;
             QCD_CUDA(c, cudaMemcpyAsync(c->h_results, c->results, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
             QCD_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -21,13 +21,18 @@ constexpr int kMaxBlocks = 148 * 16;  // grid-stride above this: a multiple of t
 // r = b ; p_k = b (all k) ; rho = rho_b = <b,b> ; x_k are zeroed by a memset
 __global__ void __launch_bounds__(kBlock)
 cg_init_kernel(long n2, const double2 *__restrict__ b, double2 *__restrict__ r,
-               double2 *__restrict__ p, long pstride, int nshift, double *partial, CgState *st)
+               double2 *__restrict__ p, long pstride, int nshift, double *partial, CgState *st,
+               int Vh, int halo)
 {
     pdl_wait();
     pdl_launch_dependents();
     double s = 0.0;
     for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
-        const double2 v = __ldg(b + i);
+        double2 v = __ldg(b + i);
+        if (halo > 0) {        // slab mode: the first and the last t-slice (halo sites each) are not this rank's
+            const int h = (int)(i % Vh);
+            if (h < halo || h >= Vh - halo) v = make_double2(0.0, 0.0);
+        }
         r[i] = v;
         for (int k = 0; k < nshift; ++k) p[k * pstride + i] = v;
         s += v.x * v.x + v.y * v.y;
@@ -55,7 +60,7 @@ constexpr int kRUnroll = 4;                       // independent 16-byte loads p
 constexpr int kRChunk = kBlock * kRUnroll;
 constexpr int kRMaxBlocks = 148 * 4;
 
-template <bool LOOP>
+template <bool LOOP, bool SPLIT = false>
 __global__ void __launch_bounds__(kBlock)
 cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
                    const double *__restrict__ pap_partial, int npap, double *partial, CgState *st,
@@ -110,6 +115,10 @@ cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
     }
     double total;
     if (grid_sum_last_block<kBlock>(s, partial, &st->counter, total)) {
+        if (SPLIT) {                      // slab mode: the sum over the ranks and the scalar step follow (api.cu)
+            if (threadIdx.x == 0) st->red[1] = total;
+            return;
+        }
         cg_step_alpha(st, pAp);
         __syncthreads();
         cg_step_beta(st, total);
@@ -563,14 +572,18 @@ add_c0_kernel(long n2, double c0, const double2 *__restrict__ b, double2 *y)
 // out = b - q ; *result = ||out||^2   (outer residual of the mixed-precision refinement, NEXT-3)
 __global__ void __launch_bounds__(kBlock)
 residual_kernel(long n2, const double2 *__restrict__ b, const double2 *__restrict__ q, double2 *__restrict__ out,
-                double *partial, unsigned *counter, double *result)
+                double *partial, unsigned *counter, double *result, int Vh, int halo)
 {
     pdl_wait();
     pdl_launch_dependents();
     double s = 0.0;
     for (long i = (long)blockIdx.x * kBlock + threadIdx.x; i < n2; i += (long)gridDim.x * kBlock) {
         const double2 bv = __ldg(b + i), qv = __ldg(q + i);
-        const double2 d = make_double2(bv.x - qv.x, bv.y - qv.y);
+        double2 d = make_double2(bv.x - qv.x, bv.y - qv.y);
+        if (halo > 0) {        // slab mode: halo slices are not this rank's
+            const int h = (int)(i % Vh);
+            if (h < halo || h >= Vh - halo) d = make_double2(0.0, 0.0);
+        }
         out[i] = d;
         s += d.x * d.x + d.y * d.y;
     }
@@ -588,9 +601,9 @@ int blas_grid_blocks(long n2)
 }
 
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
-                   double *partial, CgState *st, Launch L)
+                   double *partial, CgState *st, int Vh, int halo, Launch L)
 {
-    launch_kernel(cg_init_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, r, p, pstride, nshift, partial, st);
+    launch_kernel(cg_init_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, r, p, pstride, nshift, partial, st, Vh, halo);
     return 1;
 }
 
@@ -610,6 +623,61 @@ int launch_cg_update_r(long n2, double2 *ring, const double2 *q, const double *p
     else
         launch_kernel(cg_update_r_kernel<false>, grid, kBlock, L.s, L.pdl, n2, ring, q, pap_partial, npap, partial, st,
                       (cudaGraphConditionalHandle)0);
+    return 1;
+}
+
+namespace {
+
+__global__ void __launch_bounds__(kBlock)
+sum_partials_kernel(const double *__restrict__ partial, int n, double *out)
+{
+    double t = 0.0;
+    for (int i = threadIdx.x; i < n; i += kBlock) t += __ldcg(partial + i);
+    const double total = block_sum<kBlock>(t);
+    if (threadIdx.x == 0) *out = total;
+}
+
+__global__ void __launch_bounds__(kMaxShifts)
+cg_scalars_kernel(CgState *st)
+{
+    if (st->done) return;                 // dead iteration
+    cg_step_alpha(st, st->red[0]);
+    __syncthreads();
+    cg_step_beta(st, st->red[1]);
+}
+
+__global__ void cg_after_init_kernel(CgState *st)
+{
+    const double rho = st->rho;           // all-reduced ||b||^2
+    st->rho_b = rho;
+    st->done = st->done_prev = rho == 0.0 ? 1 : 0;
+}
+
+}  // namespace
+
+int launch_cg_update_r_split(long n2, double2 *ring, const double2 *q, const double *pap, double *partial,
+                             CgState *st, Launch L)
+{
+    launch_kernel(cg_update_r_kernel<false, true>, cg_update_r_grid_blocks(n2), kBlock, L.s, L.pdl, n2, ring, q, pap, 1,
+                  partial, st, (cudaGraphConditionalHandle)0);
+    return 1;
+}
+
+int launch_sum_partials(const double *partial, int n, double *out, Launch L)
+{
+    launch_kernel(sum_partials_kernel, 1, kBlock, L.s, L.pdl, partial, n, out);
+    return 1;
+}
+
+int launch_cg_scalars(CgState *st, Launch L)
+{
+    launch_kernel(cg_scalars_kernel, 1, kMaxShifts, L.s, L.pdl, st);
+    return 1;
+}
+
+int launch_cg_after_init(CgState *st, Launch L)
+{
+    launch_kernel(cg_after_init_kernel, 1, 1, L.s, L.pdl, st);
     return 1;
 }
 
@@ -685,9 +753,9 @@ int launch_cg_flush_shifts_y(long n2, const double2 *ring, double2 *y, double2 *
 }
 
 int launch_residual(long n2, const double2 *b, const double2 *q, double2 *out, double *partial, unsigned *counter,
-                    double *result, Launch L)
+                    double *result, int Vh, int halo, Launch L)
 {
-    launch_kernel(residual_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, q, out, partial, counter, result);
+    launch_kernel(residual_kernel, blas_grid_blocks(n2), kBlock, L.s, L.pdl, n2, b, q, out, partial, counter, result, Vh, halo);
     return 1;
 }
 

@@ -62,6 +62,7 @@ struct CgState {
     int done_prev;                // set one (dead) iteration later: gates the shift update
     unsigned counter;             // last-block-done ticket
     double scratch;               // generic reduction result (norms for true residuals)
+    double red[2];                // slab mode: <p_0,q> and ||r'||^2, summed over the rank, then over the ranks
     int not_su3;                  // set by the two-row gauge ingest (layout.cu)
     double cy[kMaxShifts];        // y-only mode: residues c_k of eq. 8 in sorted-shift order
     // deferred shift updates (blas.cu): the coefficients of the last `defer` iterations, slot (n - 1) % defer
@@ -138,7 +139,7 @@ int launch_ingest_links(const Geom &g, const double *links_canon, double2 *W, in
 int launch_ingest_links32(const Geom &g, const double *links_canon, float2 *W32, Launch L);
 // out = b - q, *result = ||out||^2 (one ticketed reduction)
 int launch_residual(long n2, const double2 *b, const double2 *q, double2 *out, double *partial, unsigned *counter,
-                    double *result, Launch L);
+                    double *result, int Vh, int halo, Launch L);   // halo as in launch_cg_init
 // sites h0 <= h < h1 only (h1 < 0: all)
 int launch_pack(const Geom &g, const double *canon, double2 *internal, Launch L, int h0 = 0, int h1 = -1);
 int launch_unpack(const Geom &g, const double2 *internal, double *canon, Launch L, int h0 = 0, int h1 = -1);
@@ -197,8 +198,9 @@ int launch_dslash_multi(const Geom &g, const DslashMultiParams &p, Launch L);
 
 // BLAS-1 (n2 = 3*Vh double2 elements per vector)
 int blas_grid_blocks(long n2);
+// halo > 0 (slab mode): the first and the last `halo` sites of every colour plane (Vh sites) are taken as zero
 int launch_cg_init(long n2, const double2 *b, double2 *r, double2 *p, long pstride, int nshift,
-                   double *partial, CgState *st, Launch L);
+                   double *partial, CgState *st, int Vh, int halo, Launch L);
 // loop_handle != 0: the kernel is a node of a WHILE conditional graph and sets its condition
 // The residual lives in a ring of st->defer vectors (stride n2): r after iteration n is slot (n - 1) % defer,
 // the initial residual b is slot defer - 1.
@@ -220,6 +222,15 @@ int launch_cg_update_shifts(long n2, const double2 *ring, double2 *x, double2 *p
 // the deferred updates of the shifts k >= 1 for the last `window` enqueued iterations, in one pass
 int launch_cg_flush_shifts(long n2, const double2 *ring, double2 *x, double2 *p, long pstride,
                            const CgState *st, int window, Launch L);
+// ---- slab (distributed) mode: the reductions leave the rank between the kernels (api.cu) ----
+// split != 0: the r-update's last block stores the rank's ||r'||^2 in st->red[1] and leaves the scalar step
+// to launch_cg_scalars (after the all-reduce)
+int launch_cg_update_r_split(long n2, double2 *ring, const double2 *q, const double *pap, double *partial,
+                             CgState *st, Launch L);
+int launch_sum_partials(const double *partial, int n, double *out, Launch L);   // *out = sum partial[0..n)
+int launch_cg_scalars(CgState *st, Launch L);        // alpha_k/zeta, beta, freeze, stop from st->red[0..1]
+int launch_cg_after_init(CgState *st, Launch L);     // rho_b = rho (all-reduced), done = (rho == 0)
+
 // y = c0 b + sum_k residues[k] x_k  (b == nullptr: no c0 term)
 int launch_combine(long n2, const double2 *x, const long long *xoff_host, const double *residues,
                    int nshift, double c0, const double2 *b, double2 *y, Launch L);

@@ -1,5 +1,6 @@
-"""t-slab decomposition of the lattice over ranks (first half): index maps and
-halo exchange only -- no operator arithmetic lives here; the stencil is qcd_dslash_range.
+"""t-slab decomposition of the lattice over ranks: index maps, halo exchange and
+the callbacks of the library's slab mode -- no operator or solver arithmetic lives here; the stencil is the
+library's (qcd_dslash_range, or qcd_dslash / qcd_mdagm / qcd_multishift_cg after qcd_set_slab).
 
 The paper slices the lattice along z, K computational slices plus halos per node, and exchanges the
 faces before every D.  Here the slicing direction is t (the slowest
@@ -27,12 +28,25 @@ global t_lo + nt_loc   (both taken modulo Nt).  Consequences, all handled here:
 A slice of an internal vector (three colour planes, site-fastest) is three contiguous runs of
 Nx/2*Ny*Nz complex numbers, 24 * Nx*Ny*Nz bytes in all: the 48 B x face sites per direction of
 SURVEY.md 8(e).  `exchange_halos` moves them with torch.distributed point-to-point calls (gloo on the
-CPU, nccl between GPUs); a device-initiated NVLink put fused into the stencil is the next step and is
-not built.
+CPU, nccl between GPUs); `attach` hands the library the two callbacks of its slab mode (halo fill, sum over
+the ranks).  A device-initiated NVLink put fused into the stencil is the next step and is not built
+(DESIGN.md section 7).
 """
 from __future__ import annotations
 
 import numpy as np
+
+
+class _DevicePointer:
+    """A device address dressed up for torch.as_tensor (zero-copy view of library-owned memory)."""
+
+    def __init__(self, ptr: int, doubles: int):
+        self.__cuda_array_interface__ = {"shape": (doubles,), "typestr": "<f8", "data": (ptr, False), "version": 3}
+
+
+def device_view(ptr: int, doubles: int):
+    import torch
+    return torch.as_tensor(_DevicePointer(ptr, doubles), device="cuda")
 
 
 class SlabPartition:
@@ -101,13 +115,16 @@ class SlabPartition:
         a = vec.view(n + 2, self.slice_half * 6)
         return a[0], a[1], a[n], a[n + 1]
 
-    def exchange_halos(self, vec, dist, internal: bool = True):
+    def exchange_halos(self, vec, dist, internal: bool = True, staged: bool = False):
         """Fill the two halo slices of `vec` (a torch tensor, one extended local parity vector) from the
         neighbouring ranks: my first owned slice becomes the upper halo of `down`, my last owned slice
-        the lower halo of `up`.  24 * Nx*Ny*Nz bytes per direction."""
+        the lower halo of `up`.  24 * Nx*Ny*Nz bytes per direction.  staged: the four slices travel through
+        host copies (a CUDA vector over the gloo backend)."""
         import torch
         lo_halo, first, last, hi_halo = self._slices(vec, internal)
         send_dn, send_up = first.contiguous(), last.contiguous()
+        if staged:
+            send_dn, send_up = send_dn.cpu(), send_up.cpu()
         recv_lo, recv_hi = torch.empty_like(send_up), torch.empty_like(send_dn)
         ops = [dist.P2POp(dist.isend, send_up, self.up), dist.P2POp(dist.irecv, recv_lo, self.down),
                dist.P2POp(dist.isend, send_dn, self.down), dist.P2POp(dist.irecv, recv_hi, self.up)]
@@ -116,3 +133,41 @@ class SlabPartition:
         lo_halo.copy_(recv_lo)
         hi_halo.copy_(recv_hi)
         return vec
+
+    # ---- the library's slab mode (qcd_set_slab): this rank's callbacks
+    def attach(self, ctx, dist, staged: bool = False):
+        """Put `ctx` (a Context on the extended local lattice `local_dims`) into slab mode with callbacks
+        that move the halo slices and sum the inner products over `dist`'s default group.
+        staged = False: the collectives act on the device buffers themselves (backend nccl, one GPU per
+        rank).  staged = True: through host copies (backend gloo; lets several ranks share ONE GPU in the
+        tests -- every callback synchronises, no kernel ever waits for another rank's kernel)."""
+        import torch
+        vd = ctx.vector_doubles
+
+        def lib_stream(handle):
+            # the library's stream as a torch stream; handle 0 is the legacy default stream, which
+            # ExternalStream(0) would NOT give (a null pointer makes torch take a fresh pool stream)
+            return torch.cuda.default_stream() if not handle else torch.cuda.ExternalStream(handle)
+
+        def halo(ptr, stream):
+            vec = device_view(ptr, vd)
+            with torch.cuda.stream(lib_stream(stream)):
+                if staged:
+                    torch.cuda.current_stream().synchronize()
+                self.exchange_halos(vec, dist, internal=True, staged=staged)
+                if staged:
+                    torch.cuda.current_stream().synchronize()
+
+        def allreduce(ptr, count, stream):
+            buf = device_view(ptr, count)
+            with torch.cuda.stream(lib_stream(stream)):
+                if not staged:
+                    dist.all_reduce(buf)
+                    return
+                torch.cuda.current_stream().synchronize()
+                host = buf.cpu()
+                dist.all_reduce(host)
+                buf.copy_(host)
+                torch.cuda.current_stream().synchronize()
+
+        ctx.set_slab(halo, allreduce)

@@ -93,8 +93,9 @@ def test_slab_decomposition_equals_the_global_operator(tmp_path, world, dims):
     port = _free_port()
     script = tmp_path / "worker.py"
     script.write_text(_WORKER.format(root=ROOT, port=port, world=world, dims=dims))
+    env = dict(os.environ, OMP_NUM_THREADS="2")     # the ranks share the host: small OpenMP teams
     procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE,
-                              stderr=subprocess.PIPE, text=True) for r in range(world)]
+                              stderr=subprocess.PIPE, text=True, env=env) for r in range(world)]
     outs = []
     for p in procs:
         o, e = p.communicate(timeout=300)

@@ -1,0 +1,132 @@
+"""the library's slab mode (qcd_set_slab) end to end -- two ranks, each holding one
+t-slab with its halo slices as a lattice of its own, exchange halos before every D and sum the CG's inner
+products over the ranks.  The lease has ONE GPU, so both ranks use it, with the gloo backend and staged
+(host-copied) callbacks: every callback synchronises, no kernel ever waits for another rank's kernel.  The
+gathered results must match the oracle's GLOBAL operator and polished solutions within the usual bars."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, {root!r})
+sys.path.insert(0, os.path.join({root!r}, "tests"))
+import numpy as np, torch
+import torch.distributed as dist
+import lattice_inputs as li
+import oracle
+import paper_1710_09178_b200 as q
+from paper_1710_09178_b200.slab import SlabPartition
+
+world = {world}
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:{port}", rank=int(sys.argv[1]), world_size=world)
+rank = dist.get_rank()
+torch.cuda.set_device(0)
+dims, mass, tol = {dims!r}, {mass!r}, 1e-10
+E, O = 0, 1
+links = li.make_links(dims, "random", 3)
+ve = li.make_source(dims, 41, E)
+shifts, res = np.array([0.3, 0.01, 1.5, 0.05]), np.array([1.0, -0.5, 2.0, 0.25])
+glob = oracle.Lattice(dims, links)
+part = SlabPartition(dims, world, rank)
+ctx = q.Context(part.local_dims, mass)
+ctx.load_gauge(torch.from_numpy(part.local_links(links)).cuda())
+part.attach(ctx, dist, staged=True)
+lE, lO = part.local_parity(E), part.local_parity(O)
+n = part.nt_loc
+
+def owned_only(v_global):          # this rank's part of a global vector, halo slices zeroed
+    a = part.local_vector(v_global).reshape(n + 2, part.slice_half, 3, 2).copy()
+    a[0] = 0.0; a[-1] = 0.0
+    return a.reshape(-1, 3, 2)
+
+def up(par, canon):
+    d = ctx.new_vector()
+    ctx.pack(par, torch.from_numpy(np.ascontiguousarray(canon)).cuda().reshape(-1), d)
+    return d
+
+def down(par, d):
+    c = torch.empty_like(d)
+    ctx.unpack(par, d, c)
+    return c.cpu().numpy().reshape(-1, 3, 2)
+
+def gather(owned):
+    parts = [torch.empty_like(torch.from_numpy(owned)) for _ in range(world)]
+    dist.all_gather(parts, torch.from_numpy(np.ascontiguousarray(owned)))
+    return np.concatenate([p.numpy() for p in parts])
+
+def rel(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+out = {{"rank": rank}}
+d_in = up(lE, owned_only(ve))
+d_o, d_a = ctx.new_vector(), ctx.new_vector()
+d_o.zero_(); d_a.zero_()
+ctx.dslash(lO, d_in, d_o)                    # global D_oe: halo of d_in filled by the callback
+out["D_oe"] = rel(gather(part.owned(down(lO, d_o))), glob.dslash(O, ve))
+ctx.mdagm(lE, d_in, d_a)
+out["MdagM"] = rel(gather(part.owned(down(lE, d_a))), glob.mdagm(mass, E, ve))
+d_x, d_y = ctx.new_vector(len(shifts)), ctx.new_vector()
+# d_in's halo slices now hold the neighbours' data (the callback wrote them): the solver must ignore them
+st, it, tr = ctx.multishift_cg(lE, d_in, shifts, res, tol, 10000, d_x, d_y)
+exact = glob.solve_exact(mass, E, ve, shifts, res, tol)
+ref = glob.multishift_cg(mass, E, ve, shifts, res, tol, want_x=False)
+out.update(status=st, iterations=it, ref_iterations=ref["iterations"], true_res=[float(t) for t in tr])
+out["x_err"] = [rel(gather(part.owned(down(lE, d_x[k]))), exact["x"][k]) for k in range(len(shifts))]
+out["y_err"] = rel(gather(part.owned(down(lE, d_y))), exact["y"])
+# residuals recomputed by the oracle's global operator from the gathered solutions
+xs = [gather(part.owned(down(lE, d_x[k]))) for k in range(len(shifts))]
+out["oracle_res"] = [float(np.linalg.norm(ve - (glob.mdagm(mass, E, xs[k]) + shifts[k] * xs[k])) / np.linalg.norm(ve))
+                     for k in range(len(shifts))]
+cut = ctx.multishift_cg(lE, d_in, shifts, res, tol, 7, d_x, d_y)
+out["cut"] = [int(cut[0]), int(cut[1])]
+dist.barrier()
+print(json.dumps(out))
+ctx.close()
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("world,dims,mass", [(2, (8, 6, 4, 8), 0.07), (4, (4, 4, 6, 8), 0.3)])   # 4 ranks: two owned slices each
+def test_slab_mode_ranks_share_one_gpu(tmp_path, world, dims, mass):
+    port = _free_port()
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT, port=port, world=world, dims=dims, mass=mass))
+    # the ranks share the host too: keep the oracle's OpenMP teams small (oversubscribed teams spin)
+    env = dict(os.environ, OMP_NUM_THREADS="2")
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE,
+                              stderr=subprocess.PIPE, text=True, env=env) for r in range(world)]
+    outs = []
+    for p in procs:
+        try:
+            o, e = p.communicate(timeout=600)
+        except subprocess.TimeoutExpired:
+            for pp in procs:
+                pp.kill()
+            raise
+        assert p.returncode == 0, e[-3000:]
+        outs.append(json.loads(o.strip().splitlines()[-1]))
+    assert sorted(o["rank"] for o in outs) == list(range(world))
+    for o in outs:
+        assert o["D_oe"] <= 1e-13 and o["MdagM"] <= 1e-13, o
+        assert o["status"] == 0 and abs(o["iterations"] - o["ref_iterations"]) <= 2, o
+        assert max(o["true_res"]) <= 1.5e-10 and max(o["x_err"]) <= 1e-9 and o["y_err"] <= 1e-9, o
+        for a, b in zip(o["true_res"], o["oracle_res"]):
+            assert abs(a - b) <= 1e-3 * b + 1e-15
+        assert o["cut"] == [4, 7]
+    # every rank ran the same iteration on replicated scalars
+    assert len({o["iterations"] for o in outs}) == 1 and len({tuple(o["true_res"]) for o in outs}) == 1
