@@ -1015,6 +1015,7 @@ qcd_status qcd_inv_sqrt(qcd_ctx *c, int parity, const double *d_phi, int n, doub
 qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, double *h_out)
 {
     if (!c) return QCD_EINVAL;
+    if (c->slab) return fail(c, QCD_EINVAL, "qcd_dslash_host: not available in slab mode (qcd_set_slab)");
     if (bad_parity(out_parity) || !h_in || !h_out)
         return fail(c, QCD_EINVAL, "qcd_dslash_host: bad argument");
     if (!c->gauge_loaded) return fail(c, QCD_ESTATE, "qcd_dslash_host: no gauge field loaded");
@@ -1085,6 +1086,7 @@ qcd_status qcd_dslash_host(qcd_ctx *c, int out_parity, const double *h_in, doubl
 qcd_status qcd_mdagm_host(qcd_ctx *c, int parity, const double *h_in, double *h_out)
 {
     if (!c) return QCD_EINVAL;
+    if (c->slab) return fail(c, QCD_EINVAL, "qcd_mdagm_host: not available in slab mode (qcd_set_slab)");
     if (bad_parity(parity) || !h_in || !h_out)
         return fail(c, QCD_EINVAL, "qcd_mdagm_host: bad argument");
     qcd_status s = ensure_host_staging(c);
@@ -1104,6 +1106,7 @@ qcd_status qcd_multishift_cg_host(qcd_ctx *c, int parity, const double *h_b, int
                                   double *true_res)
 {
     if (!c) return QCD_EINVAL;
+    if (c->slab) return fail(c, QCD_EINVAL, "qcd_multishift_cg_host: not available in slab mode (qcd_set_slab)");
     if (!h_b) return fail(c, QCD_EINVAL, "qcd_multishift_cg_host: NULL source");
     if (nshift < 1 || nshift > kMaxShifts)
         return fail(c, QCD_EINVAL, "qcd_multishift_cg_host: nshift must be in [1, QCD_MAX_SHIFTS]");
