@@ -285,6 +285,18 @@ cg_update_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__re
 #ifndef QCD_FLUSH_SHIFTS
 #define QCD_FLUSH_SHIFTS 2
 #endif
+// x_k, p_k of the deferred shifts are touched once per flush: QCD_FLUSH_STREAM = 1 loads and stores them with the
+// streaming (evict-first) policy, so that a flush does not push the links and the iteration's vectors out of L2
+#ifndef QCD_FLUSH_STREAM
+#define QCD_FLUSH_STREAM 0
+#endif
+#if QCD_FLUSH_STREAM
+#define QCD_FLUSH_LD(ptr) __ldcs(ptr)
+#define QCD_FLUSH_ST(ptr, v) __stcs(ptr, v)
+#else
+#define QCD_FLUSH_LD(ptr) (*(ptr))
+#define QCD_FLUSH_ST(ptr, v) (*(ptr) = (v))
+#endif
 constexpr int kFlushBlock = QCD_FLUSH_BLOCK;
 constexpr int kFlushShifts = QCD_FLUSH_SHIFTS;   // shifts whose x_k, p_k a thread has in flight at once
 
@@ -346,8 +358,8 @@ cg_flush_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__res
             for (int s = 0; s < kFlushShifts; ++s) {
                 steps[s] = 0;
                 if (l + s < nl) {
-                    xv[s] = x[s_x[l + s] + i];
-                    pv[s] = p[s_p[l + s] + i];
+                    xv[s] = QCD_FLUSH_LD(x + s_x[l + s] + i);
+                    pv[s] = QCD_FLUSH_LD(p + s_p[l + s] + i);
                     steps[s] = s_steps[l + s];
                 }
             }
@@ -367,8 +379,8 @@ cg_flush_shifts_kernel(long n2, const double2 *__restrict__ ring, double2 *__res
 #pragma unroll
             for (int s = 0; s < kFlushShifts; ++s) {
                 if (l + s < nl) {
-                    x[s_x[l + s] + i] = xv[s];
-                    p[s_p[l + s] + i] = pv[s];
+                    QCD_FLUSH_ST(x + s_x[l + s] + i, xv[s]);
+                    QCD_FLUSH_ST(p + s_p[l + s] + i, pv[s]);
                 }
             }
         }
