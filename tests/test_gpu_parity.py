@@ -881,6 +881,36 @@ def test_config5_full_size(torch, q):
     assert st == 0 and tr < 1e-13 and rel_l2(out["x"][15], xs) <= TOL_X
 
 
+@pytest.mark.slow
+def test_config5_two_row_links_and_bulk_kernel(torch, q):
+    """The options at the largest size: two-row link storage (NEXT-1) solves config 5 to the same stored
+    oracle solutions (base shift included), and the bulk-staged Dslash (one CTA per tile and persistent)
+    gives the bits of the register-staged one on the 2.4 GB field."""
+    cfg, links, b, shifts, res = li.make_config_inputs(5)
+    gen, gold = _golden_cfg5()
+    sites = gen.sample_sites(cfg)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links, link_rows=2)
+    ref_o = rig.lat.dslash(O, b)
+    assert rel_l2(rig.dslash(O, b), ref_o) <= TOL_OP
+    out = rig.solve(E, b, shifts, res, cfg.tol)
+    assert out["status"] == 0 and (out["true_res"] <= 1.5 * cfg.tol).all(), out["true_res"]
+    for k, g in gold.items():
+        xk = out["x"][k]
+        err = np.linalg.norm((xk[sites] - g["x"]).ravel()) / np.linalg.norm(g["x"].ravel())
+        assert err <= TOL_X, (k, err)
+        n2 = float(np.sum(xk.astype(np.longdouble) ** 2))
+        assert abs(n2 - g["norm2"]) <= 2 * TOL_X * g["norm2"], (k, n2, g["norm2"])
+    rig.ctx.close()
+    del out
+    rig3 = Rig(torch, q, cfg.dims, cfg.mass, links)
+    d3 = rig3.dslash(O, b)
+    assert rel_l2(d3, ref_o) <= TOL_OP
+    rig3.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, 1)
+    for persist in (0, 3):
+        rig3.ctx.set_option(q.QCD_OPT_DSLASH_PERSIST, persist)
+        assert np.array_equal(rig3.dslash(O, b), d3), persist
+
+
 # ------------------------------------------------------------------ (M^dag M)^(1/4) phi  (heat bath, PAPER.md:131)
 
 def test_fourth_root_matches_oracle_and_dense_definition(torch, q):
