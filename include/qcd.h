@@ -102,7 +102,7 @@ QCD_API qcd_status qcd_set_stream(qcd_ctx *ctx, void *cuda_stream);
  *                     taken in another order).  Not used by single-shift solves.
  *   QCD_OPT_CG_FUSE   (default 1) 1: the r-update and the base-shift update of an iteration run as ONE cooperative
  *                     kernel with a grid-wide barrier between them (needs QCD_OPT_CG_DEFER > 1, not used
- *                     by the y-only form and by QCD_OPT_CG_GRAPH = 2); 0: two kernels, the second
+ *                     by QCD_OPT_CG_GRAPH = 2); 0: two kernels, the second
  *                     waiting for the first's last block.  Bit-identical results.
  *   QCD_OPT_TGROUP    (default 0 = chosen by the library) order in which the Dslash CTAs walk the
  *                     lattice: groups of this many 128-site chunks of a t-slice are processed for all t

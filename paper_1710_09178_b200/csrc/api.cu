@@ -288,8 +288,9 @@ void enqueue_cg_iteration(qcd_ctx *c, int parity, double2 *x, bool y_only)
     }
     const int npap = c->opt_dslash_kernel == 1 && !c->use_links32 ? dslash_bulk_grid_blocks(c->g, c->opt_dslash_persist)
                                                : dslash_grid_blocks(c->g);
-    if (c->opt_cg_fuse && !y_only && c->cur_defer > 1 && c->loop_handle == 0) {
-        const int n = launch_cg_update_r_base(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, x, c->p, c->st, c->L());
+    if (c->opt_cg_fuse && c->cur_defer > 1 && c->loop_handle == 0) {
+        const int n = launch_cg_update_r_base(c->n2, c->r, c->q, c->pap_partial, npap, c->partial, x, c->p, c->st,
+                                              y_only ? 1 : 0, c->L());
         c->launches += n;
         if (n) return;
     }

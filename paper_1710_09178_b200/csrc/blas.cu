@@ -138,7 +138,7 @@ cg_update_r_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
 __global__ void __launch_bounds__(kBlock)
 cg_update_r_base_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
                         const double *__restrict__ pap_partial, int npap, double *partial,
-                        double2 *__restrict__ x, double2 *__restrict__ p, CgState *st)
+                        double2 *__restrict__ x, double2 *__restrict__ p, CgState *st, int y_only)
 {
     pdl_wait();
     pdl_launch_dependents();
@@ -152,7 +152,9 @@ cg_update_r_base_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
     const double rho = st->rho;
     const double2 *rin = ring + (long)((it + m - 1) % m) * n2;
     double2 *r = ring + (long)(it % m) * n2;
-    double2 *__restrict__ x0 = x + st->xoff[0];
+    // y-only form: x is the accumulator y, which takes c_0 alpha p_0 where x_0 would take alpha p_0
+    double2 *__restrict__ x0 = y_only ? x : x + st->xoff[0];
+    const double cy0 = y_only ? st->cy[0] : 1.0;
     double t = 0.0;
     for (int i = threadIdx.x; i < npap; i += kBlock) t += __ldcg(pap_partial + i);
     const double pAp = block_sum<kBlock>(t);
@@ -184,6 +186,7 @@ cg_update_r_base_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
     for (unsigned i = threadIdx.x; i < gridDim.x; i += kBlock) u += __ldcg(partial + i);
     const double rho_new = block_sum<kBlock>(u);
     const double beta = rho_new / rho;
+    const double ax = y_only ? cy0 * alpha : alpha;
     for (long base = (long)blockIdx.x * kRChunk + threadIdx.x; base < n2; base += (long)gridDim.x * kRChunk) {
         double2 rv[kRUnroll], xv[kRUnroll], pv[kRUnroll];
 #pragma unroll
@@ -195,8 +198,8 @@ cg_update_r_base_kernel(long n2, double2 *ring, const double2 *__restrict__ q,
         for (int e = 0; e < kRUnroll; ++e) {
             const long i = base + (long)e * kBlock;
             if (i < n2) {
-                xv[e].x = fma(alpha, pv[e].x, xv[e].x);
-                xv[e].y = fma(alpha, pv[e].y, xv[e].y);
+                xv[e].x = fma(ax, pv[e].x, xv[e].x);
+                xv[e].y = fma(ax, pv[e].y, xv[e].y);
                 pv[e].x = fma(beta, pv[e].x, 1.0 * rv[e].x);
                 pv[e].y = fma(beta, pv[e].y, 1.0 * rv[e].y);
                 x0[i] = xv[e];
@@ -695,7 +698,7 @@ int launch_cg_after_init(CgState *st, Launch L)
 
 // 0 if the cooperative launch is not possible (grid would not be co-resident)
 int launch_cg_update_r_base(long n2, double2 *ring, const double2 *q, const double *pap_partial, int npap,
-                            double *partial, double2 *x, double2 *p, CgState *st, Launch L)
+                            double *partial, double2 *x, double2 *p, CgState *st, int y_only, Launch L)
 {
     static int max_blocks = -1;
     if (max_blocks < 0) {
@@ -723,7 +726,7 @@ int launch_cg_update_r_base(long n2, double2 *ring, const double2 *q, const doub
     }
     cfg.attrs = attr;
     cfg.numAttrs = na;
-    cudaLaunchKernelEx(&cfg, cg_update_r_base_kernel, n2, ring, q, pap_partial, npap, partial, x, p, st);
+    cudaLaunchKernelEx(&cfg, cg_update_r_base_kernel, n2, ring, q, pap_partial, npap, partial, x, p, st, y_only);
     return 1;
 }
 

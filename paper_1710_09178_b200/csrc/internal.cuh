@@ -210,7 +210,7 @@ int launch_cg_update_r(long n2, double2 *ring, const double2 *q, const double *p
 // r-update and base-shift update in one cooperative kernel (QCD_OPT_CG_FUSE); returns 0 without launching if
 // the grid cannot be co-resident
 int launch_cg_update_r_base(long n2, double2 *ring, const double2 *q, const double *pap_partial, int npap,
-                            double *partial, double2 *x, double2 *p, CgState *st, Launch L);
+                            double *partial, double2 *x, double2 *p, CgState *st, int y_only, Launch L);
 // y-only form: y += sum_k c_k alpha_k p_k ; p_k = zeta_k r + beta_k p_k   (no x_k are kept)
 int launch_cg_update_shifts_y(long n2, const double2 *ring, double2 *y, double2 *p, long pstride,
                               CgState *st, int base_only, Launch L);

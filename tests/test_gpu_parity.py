@@ -979,6 +979,12 @@ def test_y_only_mode_gives_the_same_y_without_forming_x(torch, q, number, n):
             assert st2 == 0 and it2 == it1 and rel_l2(rig.to_canonical(E, d_c), yb) <= 1e-12
             assert np.allclose(tr2, tr1, rtol=1e-9)
         rig.ctx.set_option(q.QCD_OPT_CG_DEFER, 8)
+        # the fused cooperative BLAS-1 kernel (default) against the two-kernel path: same bits in the y-only form too
+        rig.ctx.set_option(q.QCD_OPT_CG_FUSE, 0)
+        d_c = rig.ctx.new_vector()
+        st3, it3, tr3, _ = rig.ctx.apply_pow(E, d_phi, num, den, n, xmin, xmax, tol, 100000, d_c)
+        assert st3 == 0 and it3 == it1 and np.array_equal(rig.to_canonical(E, d_c), yb) and np.array_equal(tr3, tr1)
+        rig.ctx.set_option(q.QCD_OPT_CG_FUSE, 1)
     # the inv_sqrt entry point takes the same path; the zero source still works
     st, it, tr, _ = rig.ctx.inv_sqrt(E, torch.zeros_like(d_phi), n, xmin, xmax, tol, 100, d_b)
     assert st == 0 and it == 0 and not rig.to_canonical(E, d_b).any() and not tr.any()
