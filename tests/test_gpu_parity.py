@@ -377,6 +377,39 @@ def test_slab_decomposition_on_one_gpu(torch, q, world, kernel):
     with pytest.raises(q.QcdError, match="QCD_EINVAL"):
         rigs[0].ctx.dslash_range(0, rigs[0].ctx.new_vector(), rigs[0].ctx.new_vector(), 1, nt)
 
+
+def test_dslash_range_writes_exactly_the_requested_slices(torch, q):
+    """qcd_dslash_range (the building block of the slab decomposition): for any t-range the requested
+    slices carry the bits of the full apply, with and without the fused epilogue, every other site of the
+    output keeps what it held; both kernels, both link layouts, both parities."""
+    dims, mass = (6, 4, 4, 10), 0.07
+    links = li.make_links(dims, "random", 17)
+    rng = np.random.default_rng(5)
+    for rows in (3, 2):
+        rig = Rig(torch, q, dims, mass, links, link_rows=rows)
+        st = rig.nh // dims[3]                     # sites of one parity per t-slice
+        for kernel in (0, 1):
+            rig.ctx.set_option(q.QCD_OPT_DSLASH_KERNEL, kernel)
+            for par in (O, E):
+                v, w = li.make_source(dims, 3 + par, 1 - par), li.make_source(dims, 9 + par, par)
+                full = rig.dslash(par, v)
+                d_in, d_src = rig.to_internal(1 - par, v), rig.to_internal(par, w)
+                for t0, nt in [(0, dims[3]), (0, 1), (dims[3] - 1, 1), (3, 4), tuple(int(x) for x in (rng.integers(0, 5), rng.integers(1, 6)))]:
+                    for fused in (False, True):
+                        d_out = torch.full((rig.ctx.vector_doubles,), 7.25, dtype=torch.float64, device="cuda")
+                        rig.ctx.dslash_range(par, d_in, d_out, t0, nt, d_src if fused else None, 0.3)
+                        out = rig.to_canonical(par, d_out).reshape(dims[3], st, 3, 2)
+                        want = (0.3 * w - full if fused else full).reshape(dims[3], st, 3, 2)
+                        assert np.array_equal(out[t0:t0 + nt], want[t0:t0 + nt]) or \
+                            rel_l2(out[t0:t0 + nt], want[t0:t0 + nt]) <= 1e-15, (rows, kernel, par, t0, nt, fused)
+                        mask = np.ones(dims[3], dtype=bool)
+                        mask[t0:t0 + nt] = False
+                        assert (out[mask] == 7.25).all(), (rows, kernel, par, t0, nt, fused)
+        for bad in ((-1, 2), (0, 0), (9, 2)):
+            with pytest.raises(q.QcdError, match="QCD_EINVAL"):
+                rig.ctx.dslash_range(O, d_in, rig.ctx.new_vector(), bad[0], bad[1])
+        rig.ctx.close()
+
 # ------------------------------------------------------------------ multishift CG
 
 def check_solve(rig, cfg, b, shifts, res, out, exact=None):
