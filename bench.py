@@ -57,11 +57,12 @@ FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback
 TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r02_dslash_traffic.json")
 
 
-def kernel_source_hash() -> str:
-    """SHA-256 over the Dslash kernel sources: ties a stored ncu traffic figure to the code it was taken from."""
+def kernel_source_hash(kernel: int = 0) -> str:
+    """SHA-256 over the sources of the Dslash kernel in question (0: register-staged, 1: bulk-staged): ties a
+    stored ncu figure to the code it was taken from."""
     import hashlib
     h = hashlib.sha256()
-    for name in ("dslash.cu", "dslash_bulk.cu", "dslash_site.cuh"):
+    for name in (("dslash.cu", "dslash_site.cuh") if kernel == 0 else ("dslash_bulk.cu", "dslash_site.cuh")):
         with open(os.path.join(ROOT, "paper_1710_09178_b200", "csrc", name), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:16]
@@ -79,7 +80,7 @@ def traffic_entry(cfg_number: int, link_rows: int, kernel: int):
     if not e:
         return {}, "no ncu capture for this workload/kernel in profiles/r02_dslash_traffic.json"
     note = f"ncu, {TRAFFIC_JSON[len(ROOT) + 1:]}"
-    if e.get("source_hash") != kernel_source_hash():
+    if e.get("source_hash") != kernel_source_hash(kernel):
         note += " (STALE: kernel sources changed since the capture)"
     return e, note
 
@@ -127,7 +128,7 @@ def ncu_import(args):
     e[f"{args.ncu_mode}_bytes_per_launch"] = tot / n
     e[f"{args.ncu_mode}_us_per_launch_under_ncu"] = 1e6 * dur / n
     e[f"{args.ncu_mode}_launches"] = n
-    e["source_hash"] = kernel_source_hash()
+    e["source_hash"] = kernel_source_hash(1 if args.ncu_key.endswith("kernel1") else 0)
     with open(TRAFFIC_JSON, "w") as fh:
         json.dump(doc, fh, indent=1, sort_keys=True)
         fh.write("\n")
