@@ -118,6 +118,10 @@ def test_slab_mode_ranks_share_one_gpu(tmp_path, world, dims, mass):
             for pp in procs:
                 pp.kill()
             raise
+        if p.returncode != 0 and ("busy or unavailable" in e or "exclusive" in e.lower()):
+            for pp in procs:
+                pp.kill()
+            pytest.skip("the GPU does not admit several processes (exclusive compute mode)")
         assert p.returncode == 0, e[-3000:]
         outs.append(json.loads(o.strip().splitlines()[-1]))
     assert sorted(o["rank"] for o in outs) == list(range(world))
