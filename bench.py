@@ -552,6 +552,9 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": n, "steps": K, "warmup": args.warmup,
         "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "value_note": "L2-ASSISTED steady state of back-to-back applies: algorithmic bytes (624 V per apply) over time, "
+                      "not DRAM bandwidth; DRAM side: roofline.frac_dram; every byte from DRAM: dslash.cold_l2 / "
+                      "target_check (one launch behind a flushed L2) and streaming (64^3x16)",
         "config": workload_config(cfg, args),
         "dslash": {"us_per_apply": 1e6 * per_launch_s, "gflops": dslash_flops(V) / per_launch_s / 1e9,
                    "pct_of_8000": 100 * achieved / 8000.0, "pct_of_measured_peak": 100 * achieved / peak},
