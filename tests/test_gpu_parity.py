@@ -450,6 +450,24 @@ def test_two_row_multishift_cg_configs_1_2(torch, q, number):
     check_solve(rig, cfg, b, shifts, res, out, exact)
 
 
+def test_config2_solutions_against_lapack_directly(torch, q):
+    """Independent of the oracle's CG and polish: the matrix of (M^dag M)_ee on config 2 assembled column by
+    column from the oracle's OPERATOR (pinned by closed forms), every shifted system solved by LAPACK, and
+    the GPU's x_k compared with that."""
+    from helpers import c as cplx, dense_from_operator
+    cfg, links, b, shifts, res = li.make_config_inputs(2)
+    rig = Rig(torch, q, cfg.dims, cfg.mass, links)
+    out = rig.solve(cfg.parity, b, shifts, res, cfg.tol)
+    a = dense_from_operator(lambda v: rig.lat.mdagm(cfg.mass, E, v), rig.nh)
+    bc = cplx(b).ravel()
+    y = np.zeros_like(bc)
+    for k, s in enumerate(shifts):
+        xd = np.linalg.solve(a + s * np.eye(a.shape[0]), bc)
+        y += res[k] * xd
+        assert rel_l2(cplx(out["x"][k]).ravel(), xd) <= TOL_X, k
+    assert rel_l2(cplx(out["y"]).ravel(), y) <= TOL_X
+
+
 def test_multishift_cg_is_deterministic(torch, q):
     cfg, links, b, shifts, res = li.make_config_inputs(2)
     rig = Rig(torch, q, cfg.dims, cfg.mass, links)

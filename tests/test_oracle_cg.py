@@ -133,3 +133,25 @@ def test_config2_iteration_count_is_modest():
     out = lat.multishift_cg(cfg.mass, 0, b, shifts, res, cfg.tol)
     assert out["status"] == 0 and 20 < out["iterations"] < 400
     assert (out["true_res"] <= 1.5 * cfg.tol).all()
+
+
+def test_polished_oracle_equals_lapack_on_config_2_itself():
+    """Config 2 (8^3 x 4, near-identity links, m = 0.05, 12 shifts down to 1e-5) is small enough for LAPACK:
+    the 3072 x 3072 matrix of (M^dag M)_ee is assembled column by column from the oracle's operator and every
+    shifted system solved densely.  Pins the polished oracle (C16) and the multishift recurrences at one of
+    the BASELINE.json configurations themselves, not only on 2^4 and 4^4."""
+    cfg, links, b, shifts, res = li.make_config_inputs(2)
+    lat = oracle.Lattice(cfg.dims, links)
+    a = dense_from_operator(lambda v: lat.mdagm(cfg.mass, 0, v), lat.volume // 2)
+    assert np.abs(a - a.conj().T).max() < 1e-14                       # Hermitian
+    bc = c(b).ravel()
+    n = a.shape[0]
+    exact = lat.solve_exact(cfg.mass, 0, b, shifts, res, cfg.tol)
+    out = lat.multishift_cg(cfg.mass, 0, b, shifts, res, cfg.tol)
+    y = np.zeros(n, dtype=complex)
+    for k in (0, 3, 7, 11):
+        xd = np.linalg.solve(a + shifts[k] * np.eye(n), bc)
+        assert rel_l2(c(exact["x"][k]).ravel(), xd) < 1e-12, k
+        assert rel_l2(c(out["x"][k]).ravel(), xd) < 1e-9, k
+    lam = np.linalg.eigvalsh(a)
+    assert lam.min() > cfg.mass ** 2 and lam.max() < cfg.mass ** 2 + 16.0   # m^2 <= spectrum <= m^2 + 16 (C1)
